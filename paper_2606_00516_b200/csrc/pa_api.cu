@@ -1,0 +1,447 @@
+// C-ABI layer of libpa_b200.so (include/pa.h): context, validation, planner (a1/a7), launches, timer (a8).
+// Host code only; kernels live in pa_kernels.cu.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <string>
+#include <vector>
+
+#include "../../include/pa.h"
+#include "pa_launch.h"
+
+using namespace pa;
+
+struct pa_ctx {
+    pa_config cfg{};
+    int G = 1;
+    int num_sms = 0;
+    std::string err;
+    // workspace layout (bytes from the workspace base)
+    int64_t off_counters = 0, off_plan = 0, off_part_ml = 0, off_part_o = 0, ws_bytes = 0;
+    int64_t plan_region_bytes = 0;
+    int32_t max_items = 0, max_bundles = 0, max_tiles = 0, max_split = 0, max_workers = 0;
+    // pinned staging for the plan upload
+    uint8_t* h_stage = nullptr;
+    cudaEvent_t stage_ev = nullptr;
+    bool stage_pending = false;
+    // current plan
+    bool planned = false;
+    PlanView view{};
+    int32_t decode_ctas = 0, n_simple_tiles = 0, launches_per_call = 0, prefill_ctas = 0;
+    // tensor-map cache
+    const void* tm_k_ptr = nullptr;
+    const void* tm_v_ptr = nullptr;
+    CUtensorMap tmK{}, tmV{};
+    // timer
+    cudaEvent_t t0 = nullptr, t1 = nullptr;
+    std::map<int, std::map<int, std::vector<double>>> samples;  // r per-mille -> n_tok -> seconds
+};
+
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn g_encode = nullptr;
+bool g_configured = false;
+
+int32_t fail(pa_ctx* ctx, int32_t code, const std::string& msg) {
+    if (ctx) ctx->err = msg;
+    return code;
+}
+int32_t cuda_fail(pa_ctx* ctx, cudaError_t e, const char* where) {
+    return fail(ctx, PA_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+
+int env_int(const char* name, int dflt) {
+    const char* v = std::getenv(name);
+    return v && *v ? std::atoi(v) : dflt;
+}
+
+// pool[num_blocks][Hkv][16][D] bf16 -> 4-D tensor map, box = 64 columns x 16 tokens of one (block, head), 128B swizzle
+int32_t make_pool_map(pa_ctx* ctx, const void* pool, CUtensorMap* out) {
+    if (!g_encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || !fn) return fail(ctx, PA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+        g_encode = reinterpret_cast<EncodeTiledFn>(fn);
+    }
+    const pa_config& c = ctx->cfg;
+    const cuuint64_t D = c.head_dim, Hkv = c.num_kv_heads;
+    cuuint64_t dims[4] = {D, (cuuint64_t)kBlock, Hkv, (cuuint64_t)c.num_blocks};
+    cuuint64_t strides[3] = {D * 2, (cuuint64_t)kBlock * D * 2, Hkv * kBlock * D * 2};
+    cuuint32_t box[4] = {64, (cuuint32_t)kBlock, 1, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = g_encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(pool), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(ctx, PA_ERR_CUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
+    return PA_OK;
+}
+
+double median(std::vector<double> v) {
+    std::sort(v.begin(), v.end());
+    size_t n = v.size();
+    return n % 2 ? v[n / 2] : 0.5 * (v[n / 2 - 1] + v[n / 2]);
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t pa_create(pa_ctx** out, const pa_config* cfg) {
+    if (!out || !cfg) return PA_ERR_INVALID;
+    *out = nullptr;
+    if (cfg->num_q_heads <= 0 || cfg->num_kv_heads <= 0 || cfg->num_blocks <= 0 || cfg->max_seqs <= 0 ||
+        cfg->max_tokens <= 0 || cfg->max_blocks_per_seq <= 0 || cfg->device < 0)
+        return PA_ERR_INVALID;
+    if ((cfg->head_dim != 128 && cfg->head_dim != 256) || cfg->block_size != kBlock ||
+        cfg->num_q_heads % cfg->num_kv_heads != 0 || cfg->num_q_heads / cfg->num_kv_heads > kMaxGroup)
+        return PA_ERR_UNSUPPORTED;
+    pa_ctx* ctx = new pa_ctx();
+    ctx->cfg = *cfg;
+    ctx->G = cfg->num_q_heads / cfg->num_kv_heads;
+    cudaError_t e = cudaSetDevice(cfg->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, cfg->device);
+    int cc_major = 0;
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, cfg->device);
+    if (e != cudaSuccess || cc_major != 10) {
+        delete ctx;
+        return PA_ERR_CUDA;  // no usable sm_100 device: there is no fallback path
+    }
+    if (!g_configured) {
+        e = configure_kernels();
+        if (e != cudaSuccess) { delete ctx; return PA_ERR_CUDA; }
+        g_configured = true;
+    }
+    // ---- workspace layout
+    ctx->max_workers = ctx->num_sms * kDecodeWarps;
+    ctx->max_bundles = ctx->max_workers * 4 + 8;
+    ctx->max_items = cfg->max_seqs * cfg->num_kv_heads + ctx->max_bundles + 8;
+    ctx->max_split = 2 * ctx->max_bundles;
+    ctx->max_tiles = cfg->max_tokens / kQTile + cfg->max_seqs + 1;
+    int64_t off = 0;
+    ctx->off_counters = off;
+    off += align_up(16 * 4 + (int64_t)cfg->max_seqs * cfg->num_kv_heads * 4, 256);
+    ctx->off_plan = off;
+    ctx->plan_region_bytes = align_up((int64_t)ctx->max_items * sizeof(DecItem), 256) +
+                             align_up((int64_t)(ctx->max_bundles + 1) * 4, 256) +
+                             align_up((int64_t)ctx->max_tiles * sizeof(PreTile), 256);
+    off += ctx->plan_region_bytes;
+    ctx->off_part_ml = off;
+    off += align_up((int64_t)ctx->max_split * kMaxGroup * sizeof(float2), 256);
+    ctx->off_part_o = off;
+    off += align_up((int64_t)ctx->max_split * ctx->G * cfg->head_dim * 4, 256);
+    ctx->ws_bytes = off;
+    e = cudaMallocHost(reinterpret_cast<void**>(&ctx->h_stage), (size_t)ctx->plan_region_bytes);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->stage_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreate(&ctx->t0);
+    if (e == cudaSuccess) e = cudaEventCreate(&ctx->t1);
+    if (e != cudaSuccess) {
+        pa_destroy(ctx);
+        return PA_ERR_CUDA;
+    }
+    *out = ctx;
+    return PA_OK;
+}
+
+int32_t pa_destroy(pa_ctx* ctx) {
+    if (!ctx) return PA_ERR_INVALID;
+    if (ctx->stage_pending && ctx->stage_ev) cudaEventSynchronize(ctx->stage_ev);
+    if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
+    if (ctx->stage_ev) cudaEventDestroy(ctx->stage_ev);
+    if (ctx->t0) cudaEventDestroy(ctx->t0);
+    if (ctx->t1) cudaEventDestroy(ctx->t1);
+    delete ctx;
+    return PA_OK;
+}
+
+int64_t pa_workspace_bytes(const pa_ctx* ctx) { return ctx ? ctx->ws_bytes : PA_ERR_INVALID; }
+
+int64_t pa_kv_pool_bytes(const pa_ctx* ctx) {
+    if (!ctx) return PA_ERR_INVALID;
+    return ctx->cfg.num_blocks * ctx->cfg.num_kv_heads * (int64_t)kBlock * ctx->cfg.head_dim * 2;
+}
+
+const char* pa_last_error(const pa_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int32_t pa_kv_append(pa_ctx* ctx, const void* k_new, const void* v_new, void* k_pool, void* v_pool,
+                     const int32_t* d_cu, const int32_t* d_ctx, const int32_t* d_bt, int32_t n_seq, int32_t n_tok,
+                     void* stream) {
+    if (!ctx) return PA_ERR_INVALID;
+    if (n_seq < 0 || n_tok < 0) return fail(ctx, PA_ERR_INVALID, "pa_kv_append: negative size");
+    if (n_seq == 0 || n_tok == 0) return PA_OK;
+    if (!k_new || !v_new || !k_pool || !v_pool || !d_cu || !d_ctx || !d_bt)
+        return fail(ctx, PA_ERR_INVALID, "pa_kv_append: null pointer");
+    if (n_seq > ctx->cfg.max_seqs || n_tok > ctx->cfg.max_tokens)
+        return fail(ctx, PA_ERR_INVALID, "pa_kv_append: n_seq/n_tok exceed the configured maxima");
+    LaunchShape sh{ctx->cfg.num_q_heads, ctx->cfg.num_kv_heads, ctx->cfg.head_dim, ctx->cfg.max_blocks_per_seq};
+    cudaError_t e = launch_kv_append(sh, k_new, v_new, k_pool, v_pool, d_cu, d_ctx, d_bt, n_seq, n_tok,
+                                     static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? PA_OK : cuda_fail(ctx, e, "pa_kv_append");
+}
+
+int32_t pa_kv_gather(pa_ctx* ctx, const void* k_pool, const void* v_pool, const int32_t* d_row, int32_t kv_len,
+                     void* k_out, void* v_out, void* stream) {
+    if (!ctx) return PA_ERR_INVALID;
+    if (kv_len < 0) return fail(ctx, PA_ERR_INVALID, "pa_kv_gather: negative kv_len");
+    if (kv_len == 0) return PA_OK;
+    if (!k_pool || !v_pool || !d_row || !k_out || !v_out) return fail(ctx, PA_ERR_INVALID, "pa_kv_gather: null pointer");
+    if (kv_len > (int64_t)ctx->cfg.max_blocks_per_seq * kBlock)
+        return fail(ctx, PA_ERR_INVALID, "pa_kv_gather: kv_len exceeds max_blocks_per_seq * 16");
+    LaunchShape sh{ctx->cfg.num_q_heads, ctx->cfg.num_kv_heads, ctx->cfg.head_dim, ctx->cfg.max_blocks_per_seq};
+    cudaError_t e = launch_kv_gather(sh, k_pool, v_pool, d_row, kv_len, k_out, v_out, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? PA_OK : cuda_fail(ctx, e, "pa_kv_gather");
+}
+
+// ---------------------------------------------------------------------------------------------
+// a1 plan.  Decode: the blocks of all (decode seq, KV head) groups form one stream that is cut into
+// equal-cost bundles (k per persistent worker; k grows with the batch so that the split partials stay
+// <= ~1 % of the KV bytes); a group cut by a bundle boundary becomes several items whose partials the
+// last-arriving worker merges.  Prefill: 128-row query tiles.
+// ---------------------------------------------------------------------------------------------
+int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t n_seq, int32_t num_decode_seqs,
+                void* d_workspace, int64_t workspace_bytes, void* stream_) {
+    if (!ctx) return PA_ERR_INVALID;
+    ctx->planned = false;
+    const pa_config& c = ctx->cfg;
+    if (n_seq < 0 || num_decode_seqs < 0 || num_decode_seqs > n_seq)
+        return fail(ctx, PA_ERR_INVALID, "pa_plan: bad n_seq / num_decode_seqs");
+    if (n_seq > c.max_seqs) return fail(ctx, PA_ERR_INVALID, "pa_plan: n_seq > max_seqs");
+    if (n_seq > 0 && (!h_cu || !h_ctx)) return fail(ctx, PA_ERR_INVALID, "pa_plan: null descriptor");
+    if (!d_workspace || workspace_bytes < ctx->ws_bytes || (reinterpret_cast<uintptr_t>(d_workspace) & 255))
+        return fail(ctx, PA_ERR_WORKSPACE, "pa_plan: workspace missing, misaligned or smaller than pa_workspace_bytes");
+    if (n_seq > 0 && h_cu[0] != 0) return fail(ctx, PA_ERR_INVALID, "pa_plan: cu_seqlens_q[0] != 0");
+    for (int s = 0; s < n_seq; ++s) {
+        const int64_t ql = (int64_t)h_cu[s + 1] - h_cu[s];
+        if (ql < 0) return fail(ctx, PA_ERR_INVALID, "pa_plan: cu_seqlens_q not non-decreasing");
+        if (h_ctx[s] < 0) return fail(ctx, PA_ERR_INVALID, "pa_plan: negative context length");
+        if (s < num_decode_seqs && ql != 1) return fail(ctx, PA_ERR_INVALID, "pa_plan: decode sequence with q_len != 1");
+        if ((int64_t)h_ctx[s] + ql > (int64_t)c.max_blocks_per_seq * kBlock)
+            return fail(ctx, PA_ERR_INVALID, "pa_plan: kv_len exceeds max_blocks_per_seq * 16");
+    }
+    const int32_t n_tok = n_seq > 0 ? h_cu[n_seq] : 0;
+    if (n_tok > c.max_tokens) return fail(ctx, PA_ERR_INVALID, "pa_plan: n_tok > max_tokens");
+
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    if (ctx->stage_pending) {
+        cudaError_t e = cudaEventSynchronize(ctx->stage_ev);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "pa_plan(stage sync)");
+        ctx->stage_pending = false;
+    }
+    const bool simple_all = (c.flags & PA_FLAG_DEBUG_SIMPLE) != 0;
+    const int Hkv = c.num_kv_heads, D = c.head_dim, G = ctx->G;
+
+    // ---- decode bundles
+    DecItem* items = reinterpret_cast<DecItem*>(ctx->h_stage);
+    int32_t n_items = 0, n_bundles = 0, n_split = 0;
+    std::vector<int32_t> bundle_start;
+    const int n_dec = simple_all ? 0 : num_decode_seqs;
+    int64_t total_blocks = 0;
+    for (int s = 0; s < n_dec; ++s) total_blocks += ((int64_t)h_ctx[s] + 1 + kBlock - 1) / kBlock * Hkv;
+    if (total_blocks > 0) {
+        const int64_t W = ctx->max_workers;
+        const double kv_bytes = (double)total_blocks * kBlock * D * 2 * 2;
+        const double part_bytes = (double)G * D * 4 * 2;
+        int k = (int)std::floor(0.01 * kv_bytes / ((double)W * part_bytes));
+        k = std::max(1, std::min(4, k));
+        k = std::max(1, std::min(4, env_int("PA_BUNDLE_K", k)));
+        const int64_t min_blocks = std::max(1, env_int("PA_MIN_BUNDLE_BLOCKS", 2));
+        const int64_t target = std::max(min_blocks, (total_blocks + W * k - 1) / (W * k));
+        bundle_start.reserve((size_t)(total_blocks / target + 2));
+        int64_t cur = 0;
+        bundle_start.push_back(0);
+        for (int s = 0; s < n_dec; ++s) {
+            const int32_t kv_len = h_ctx[s] + 1;
+            const int32_t nblk = (kv_len + kBlock - 1) / kBlock;
+            for (int g = 0; g < Hkv; ++g) {
+                int32_t pos = 0, first_item = n_items;
+                while (pos < nblk) {
+                    const int32_t take = (int32_t)std::min<int64_t>(nblk - pos, target - cur);
+                    if (n_items >= ctx->max_items) return fail(ctx, PA_ERR_INVALID, "pa_plan: decode item list overflow");
+                    items[n_items++] = DecItem{s, g, pos, pos + take, kv_len, -1, 0, 1};
+                    pos += take;
+                    cur += take;
+                    if (cur == target) {
+                        bundle_start.push_back(n_items);
+                        cur = 0;
+                    }
+                }
+                const int32_t parts = n_items - first_item;
+                if (parts > 1) {
+                    if (n_split + parts > ctx->max_split) return fail(ctx, PA_ERR_INVALID, "pa_plan: partial slots overflow");
+                    for (int32_t i = 0; i < parts; ++i) {
+                        items[first_item + i].part_base = n_split;
+                        items[first_item + i].part_idx = i;
+                        items[first_item + i].n_parts = parts;
+                    }
+                    n_split += parts;
+                }
+            }
+        }
+        if (bundle_start.back() != n_items) bundle_start.push_back(n_items);
+        n_bundles = (int32_t)bundle_start.size() - 1;
+        if (n_bundles > ctx->max_bundles) return fail(ctx, PA_ERR_INVALID, "pa_plan: bundle list overflow");
+    }
+    // ---- prefill tiles
+    int64_t off_b = align_up((int64_t)n_items * sizeof(DecItem), 256);
+    int32_t* h_bundles = reinterpret_cast<int32_t*>(ctx->h_stage + off_b);
+    for (int32_t i = 0; i <= n_bundles && n_bundles > 0; ++i) h_bundles[i] = bundle_start[i];
+    int64_t off_t = off_b + align_up((int64_t)(n_bundles + 1) * 4, 256);
+    PreTile* tiles = reinterpret_cast<PreTile*>(ctx->h_stage + off_t);
+    int32_t n_tiles = 0;
+    for (int s = simple_all ? 0 : num_decode_seqs; s < n_seq; ++s) {
+        const int32_t ql = h_cu[s + 1] - h_cu[s];
+        for (int32_t q0 = 0; q0 < ql; q0 += kQTile) {
+            if (n_tiles >= ctx->max_tiles) return fail(ctx, PA_ERR_INVALID, "pa_plan: tile list overflow");
+            tiles[n_tiles++] = PreTile{s, q0, std::min(kQTile, ql - q0), h_ctx[s]};
+        }
+    }
+    const int64_t used = off_t + align_up((int64_t)n_tiles * sizeof(PreTile), 256);
+
+    // ---- upload
+    uint8_t* ws = static_cast<uint8_t*>(d_workspace);
+    cudaError_t e = cudaMemsetAsync(ws + ctx->off_counters, 0, (size_t)(ctx->off_plan - ctx->off_counters), stream);
+    if (e == cudaSuccess && used > 0)
+        e = cudaMemcpyAsync(ws + ctx->off_plan, ctx->h_stage, (size_t)used, cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->stage_ev, stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "pa_plan(upload)");
+    ctx->stage_pending = true;
+
+    PlanView& v = ctx->view;
+    v.queue = reinterpret_cast<int32_t*>(ws + ctx->off_counters);
+    v.group_counters = v.queue + 16;
+    v.items = reinterpret_cast<const DecItem*>(ws + ctx->off_plan);
+    v.bundle_start = reinterpret_cast<const int32_t*>(ws + ctx->off_plan + off_b);
+    v.tiles = reinterpret_cast<const PreTile*>(ws + ctx->off_plan + off_t);
+    v.part_ml = reinterpret_cast<float2*>(ws + ctx->off_part_ml);
+    v.part_o = reinterpret_cast<float*>(ws + ctx->off_part_o);
+    v.n_items = n_items;
+    v.n_bundles = n_bundles;
+    v.n_tiles = n_tiles;
+    v.n_split = n_split;
+    ctx->decode_ctas = n_bundles > 0 ? std::min(ctx->num_sms, n_bundles) : 0;
+    ctx->n_simple_tiles = n_tiles;
+    ctx->prefill_ctas = 0;
+    ctx->launches_per_call = (ctx->decode_ctas > 0) + (n_tiles > 0);
+    ctx->planned = true;
+    return PA_OK;
+}
+
+int32_t pa_batch_attention(pa_ctx* ctx, const void* q, const void* k_pool, const void* v_pool, const int32_t* d_cu,
+                           const int32_t* d_ctx, const int32_t* d_bt, float softmax_scale, void* out, void* stream) {
+    if (!ctx) return PA_ERR_INVALID;
+    if (!ctx->planned) return fail(ctx, PA_ERR_INVALID, "pa_batch_attention: no valid pa_plan");
+    if (ctx->view.n_bundles == 0 && ctx->view.n_tiles == 0) return PA_OK;  // empty batch
+    if (!q || !k_pool || !v_pool || !d_cu || !d_ctx || !d_bt || !out)
+        return fail(ctx, PA_ERR_INVALID, "pa_batch_attention: null pointer");
+    if (!(softmax_scale > 0.f) || !std::isfinite(softmax_scale))
+        return fail(ctx, PA_ERR_INVALID, "pa_batch_attention: softmax_scale must be positive and finite");
+    if (ctx->tm_k_ptr != k_pool) {
+        int32_t rc = make_pool_map(ctx, k_pool, &ctx->tmK);
+        if (rc != PA_OK) return rc;
+        ctx->tm_k_ptr = k_pool;
+    }
+    if (ctx->tm_v_ptr != v_pool) {
+        int32_t rc = make_pool_map(ctx, v_pool, &ctx->tmV);
+        if (rc != PA_OK) return rc;
+        ctx->tm_v_ptr = v_pool;
+    }
+    AttnLaunch a;
+    a.sh = LaunchShape{ctx->cfg.num_q_heads, ctx->cfg.num_kv_heads, ctx->cfg.head_dim, ctx->cfg.max_blocks_per_seq};
+    a.q = q; a.out = out; a.k_pool = k_pool; a.v_pool = v_pool;
+    a.cu_seqlens_q = d_cu; a.context_lens = d_ctx; a.block_tables = d_bt;
+    a.softmax_scale = softmax_scale;
+    a.plan = ctx->view;
+    a.decode_ctas = ctx->decode_ctas;
+    a.n_simple_tiles = ctx->n_simple_tiles;
+    a.tmK = &ctx->tmK; a.tmV = &ctx->tmV;
+    int launches = 0;
+    cudaError_t e = launch_attention(a, static_cast<cudaStream_t>(stream), &launches);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "pa_batch_attention");
+    return PA_OK;
+}
+
+int64_t pa_plan_info(const pa_ctx* ctx, int32_t which) {
+    if (!ctx || !ctx->planned) return PA_ERR_INVALID;
+    switch (which) {
+        case 0: return ctx->view.n_items;
+        case 1: return ctx->view.n_bundles;
+        case 2: return ctx->view.n_split;
+        case 3: return ctx->view.n_tiles;
+        case 4: return ctx->decode_ctas + ctx->prefill_ctas;
+        case 5: return ctx->launches_per_call;
+        case 6: return ctx->prefill_ctas;
+        default: return PA_ERR_INVALID;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a8 step timer and OLS fit  T = alpha + beta * n_tok  (R^2 per PAPER.md:L439)
+// ---------------------------------------------------------------------------------------------
+int32_t pa_timer_begin(pa_ctx* ctx, void* stream) {
+    if (!ctx) return PA_ERR_INVALID;
+    cudaError_t e = cudaEventRecord(ctx->t0, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? PA_OK : cuda_fail(ctx, e, "pa_timer_begin");
+}
+
+int32_t pa_timer_record(pa_ctx* ctx, double r, int32_t n_tok, double seconds) {
+    if (!ctx) return PA_ERR_INVALID;
+    if (!(r >= 0.0 && r <= 1.0) || n_tok < 0 || !(seconds >= 0.0)) return fail(ctx, PA_ERR_INVALID, "pa_timer_record: bad sample");
+    ctx->samples[(int)std::floor(r * 1000.0 + 0.5)][n_tok].push_back(seconds);
+    return PA_OK;
+}
+
+int32_t pa_timer_end(pa_ctx* ctx, void* stream, double r, int32_t n_tok, double* seconds_out) {
+    if (!ctx) return PA_ERR_INVALID;
+    cudaError_t e = cudaEventRecord(ctx->t1, static_cast<cudaStream_t>(stream));
+    if (e == cudaSuccess) e = cudaEventSynchronize(ctx->t1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, ctx->t0, ctx->t1);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "pa_timer_end");
+    const double sec = (double)ms * 1e-3;
+    if (seconds_out) *seconds_out = sec;
+    return pa_timer_record(ctx, r, n_tok, sec);
+}
+
+int32_t pa_timer_fit(pa_ctx* ctx, double r, double* alpha, double* beta, double* r2, int32_t* n_points) {
+    if (!ctx || !alpha || !beta || !r2) return PA_ERR_INVALID;
+    auto it = ctx->samples.find((int)std::floor(r * 1000.0 + 0.5));
+    const int32_t n = it == ctx->samples.end() ? 0 : (int32_t)it->second.size();
+    if (n_points) *n_points = n;
+    if (n < 2) return fail(ctx, PA_ERR_TIMER, "pa_timer_fit: fewer than 2 distinct n_tok for this r");
+    std::vector<double> x, y;
+    for (auto& kv : it->second) {
+        x.push_back((double)kv.first);
+        y.push_back(median(kv.second));
+    }
+    double xb = 0, yb = 0;
+    for (int i = 0; i < n; ++i) { xb += x[i]; yb += y[i]; }
+    xb /= n; yb /= n;
+    double sxx = 0, sxy = 0;
+    for (int i = 0; i < n; ++i) { sxx += (x[i] - xb) * (x[i] - xb); sxy += (x[i] - xb) * (y[i] - yb); }
+    const double b = sxy / sxx, a = yb - b * xb;
+    double ss_res = 0, ss_tot = 0;
+    for (int i = 0; i < n; ++i) {
+        const double e = y[i] - (a + b * x[i]);
+        ss_res += e * e;
+        ss_tot += (y[i] - yb) * (y[i] - yb);
+    }
+    *alpha = a;
+    *beta = b;
+    *r2 = ss_tot == 0.0 ? (ss_res == 0.0 ? 1.0 : 0.0) : 1.0 - ss_res / ss_tot;
+    return PA_OK;
+}
+
+int32_t pa_timer_reset(pa_ctx* ctx) {
+    if (!ctx) return PA_ERR_INVALID;
+    ctx->samples.clear();
+    return PA_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,45 @@
+// Host-callable launch wrappers (defined in pa_kernels.cu) used by the C-ABI layer (pa_api.cu).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cstdint>
+
+#include "pa_internal.h"
+
+namespace pa {
+
+struct LaunchShape {
+    int32_t Hq, Hkv, D;
+    int32_t max_blocks_per_seq;
+};
+
+cudaError_t launch_kv_append(const LaunchShape& sh, const void* k_new, const void* v_new, void* k_pool, void* v_pool,
+                             const int32_t* cu_seqlens_q, const int32_t* context_lens, const int32_t* block_tables,
+                             int32_t n_seq, int32_t n_tok, cudaStream_t stream);
+
+cudaError_t launch_kv_gather(const LaunchShape& sh, const void* k_pool, const void* v_pool, const int32_t* table_row,
+                             int32_t kv_len, void* k_out, void* v_out, cudaStream_t stream);
+
+struct AttnLaunch {
+    LaunchShape sh;
+    const void* q;
+    void* out;
+    const void* k_pool;
+    const void* v_pool;
+    const int32_t* cu_seqlens_q;
+    const int32_t* context_lens;
+    const int32_t* block_tables;
+    float softmax_scale;
+    PlanView plan;
+    int32_t decode_ctas;     // CTAs with the decode role (0 = none)
+    int32_t n_simple_tiles;  // tiles routed to the plain kernel (v0 prefill / debug)
+    const CUtensorMap* tmK;  // host copies of the pool tensor maps
+    const CUtensorMap* tmV;
+};
+
+// Set opt-in shared memory sizes once per process/device.
+cudaError_t configure_kernels();
+cudaError_t launch_attention(const AttnLaunch& a, cudaStream_t stream, int* launches_out);
+int decode_smem_bytes(int D);
+
+}  // namespace pa

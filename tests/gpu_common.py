@@ -1,0 +1,83 @@
+"""Shared plumbing of the -m gpu parity tests: run the CUDA path through the C-ABI binding and the
+oracle on the same seeded inputs.  Imports both sides — allowed only under tests/."""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+import oracle
+from paper_2606_00516_b200 import binding
+from paper_2606_00516_b200.synth import device as sdev
+from paper_2606_00516_b200.synth import gen
+from tests import helpers
+
+MAX_ABS, MEAN_ABS = 2e-2, 2e-3     # north_star tolerance: bf16 in, fp32 accumulate, bf16 out
+
+
+def bf16_tensor(bits: np.ndarray, dev="cuda:0") -> torch.Tensor:
+    return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).to(dev).view(torch.bfloat16)
+
+
+def make_ctx(batch, flags=0, max_tokens=None):
+    sh = batch.shape
+    return binding.PagedAttention(sh.num_q_heads, sh.num_kv_heads, sh.head_dim, batch.num_blocks,
+                                  max_seqs=max(1, batch.n_seq), max_tokens=max(1, max_tokens or batch.n_tok),
+                                  max_blocks_per_seq=batch.max_blocks_per_seq, flags=flags)
+
+
+def nan_fill_device(batch, pool: torch.Tensor):
+    """Overwrite every slot that holds no cached context with the NaN sentinel (R8)."""
+    invalid = torch.from_numpy(~helpers.slot_valid_mask(batch, "ctx")).to(pool.device)     # [nb, 16]
+    pool.view(torch.int16).masked_fill_(invalid[:, None, :, None], int(np.int16(np.uint16(0x7FC0).view(np.int16))))
+
+
+def run_gpu(batch, inp=None, flags=0, repeat=1, pa=None):
+    """append + plan + attention through the C ABI.  ``inp`` = host_inputs dict (small cases) or None
+    (device fill + NaN sentinel).  Returns dict of device tensors + the context."""
+    dev = "cuda:0"
+    if inp is not None:
+        d = dict(q=bf16_tensor(inp["q"]), k_new=bf16_tensor(inp["k_new"]), v_new=bf16_tensor(inp["v_new"]),
+                 k_pool=bf16_tensor(inp["k_pool"]), v_pool=bf16_tensor(inp["v_pool"]))
+    else:
+        db = sdev.materialise(batch, dev)
+        nan_fill_device(batch, db.k_pool)
+        nan_fill_device(batch, db.v_pool)
+        d = dict(q=db.q, k_new=db.k_new, v_new=db.v_new, k_pool=db.k_pool, v_pool=db.v_pool)
+    d["pool_before"] = (d["k_pool"].clone(), d["v_pool"].clone()) if batch.pool_elems() <= (1 << 29) else None
+    cu = torch.from_numpy(batch.cu_seqlens_q).to(dev)
+    cl = torch.from_numpy(batch.context_lens).to(dev)
+    bt = torch.from_numpy(np.ascontiguousarray(batch.block_tables)).to(dev)
+    own = pa is None
+    pa = pa or make_ctx(batch, flags)
+    out = torch.full_like(d["q"], float("nan"))
+    pa.kv_append(d["k_new"], d["v_new"], d["k_pool"], d["v_pool"], cu, cl, bt, batch.n_seq, batch.n_tok)
+    pa.plan(batch.cu_seqlens_q, batch.context_lens, batch.n_seq, batch.num_decode_seqs)
+    for _ in range(repeat):
+        out.fill_(float("nan"))
+        pa.batch_attention(d["q"], d["k_pool"], d["v_pool"], cu, cl, bt, batch.softmax_scale, out)
+    torch.cuda.synchronize()
+    d.update(out=out, cu=cu, cl=cl, bt=bt, pa=pa, own=own)
+    return d
+
+
+def oracle_shape(batch):
+    sh = batch.shape
+    return oracle.PagedShape(sh.num_q_heads, sh.num_kv_heads, sh.head_dim, sh.block_size)
+
+
+def run_oracle(batch, inp, rows=None, n_threads=8):
+    osh = oracle_shape(batch)
+    kp, vp = inp["k_pool"].copy(), inp["v_pool"].copy()
+    oracle.kv_append(osh, inp["k_new"], inp["v_new"], kp, vp, batch.cu_seqlens_q, batch.context_lens, batch.block_tables)
+    ref = oracle.attention(osh, inp["q"], kp, vp, batch.cu_seqlens_q, batch.context_lens, batch.block_tables,
+                           batch.softmax_scale, rows=rows, n_threads=n_threads)
+    return ref, kp, vp
+
+
+def check_close(out_bits: np.ndarray, ref: np.ndarray, what=""):
+    got = gen.bf16_to_f64(out_bits)
+    assert np.isfinite(got).all(), f"{what}: non-finite outputs ({np.count_nonzero(~np.isfinite(got))})"
+    err = np.abs(got - ref)
+    assert err.max() <= MAX_ABS, f"{what}: max abs err {err.max():.4g} > {MAX_ABS} at {np.unravel_index(err.argmax(), err.shape)}"
+    assert err.mean() <= MEAN_ABS, f"{what}: mean abs err {err.mean():.4g} > {MEAN_ABS}"
+    return float(err.max()), float(err.mean())

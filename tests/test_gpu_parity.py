@@ -1,0 +1,210 @@
+"""-m gpu parity tests: the CUDA path through the C ABI vs the fp64 oracle on the same seeded inputs.
+
+Bar (north_star): kv_append placement and block-table gathers bit-exact; attention max abs error
+<= 2e-2 and mean abs error <= 2e-3 (bf16 in, fp32 accumulate, bf16 out).  Every pool slot that holds
+no cached context is a NaN sentinel and every unused table entry is -1 (R8), so a stray read or a
+missed append poisons the output.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_00516_b200 import binding
+from paper_2606_00516_b200.synth import device as sdev
+from paper_2606_00516_b200.synth import gen, workloads
+from tests import gpu_common as gc
+from tests import helpers
+
+pytestmark = pytest.mark.gpu
+
+
+def _small_case(name):
+    W = workloads
+    if name == "C1":
+        return W.config1()
+    if name == "ragged-tiny":
+        return W.random_batch(201, W.TINY, n_decode=9, n_prefill=4, max_ctx=300, max_q=150)
+    if name == "ragged-g4-d128":
+        return W.random_batch(202, W.QWEN3_4B, n_decode=17, n_prefill=3, max_ctx=700, max_q=260)
+    if name == "ragged-g8-d128":
+        return W.random_batch(203, W.QWEN3_30B_A3B, n_decode=11, n_prefill=2, max_ctx=500, max_q=130)
+    if name == "ragged-g4-d256":
+        return W.random_batch(204, W.GEMMA3_1B, n_decode=13, n_prefill=3, max_ctx=900, max_q=140)
+    if name == "ragged-g1-d128":
+        return W.random_batch(205, W.Shape(4, 4, 128), n_decode=7, n_prefill=2, max_ctx=200, max_q=70)
+    if name == "edge-lens":     # kv_len in {1, 15, 16, 17, 33, 128, 129}
+        return W.make_batch("edge", W.TINY, 206, [1, 1, 1, 1, 1, 1, 1, 17, 1, 128, 129],
+                            [0, 14, 15, 16, 32, 127, 128, 16, 0, 0, 127], 7)
+    if name == "decode-only":
+        return W.random_batch(207, W.QWEN3_8B, n_decode=64, n_prefill=0, max_ctx=2000, max_q=1)
+    if name == "prefill-only":
+        return W.random_batch(208, W.QWEN3_8B, n_decode=0, n_prefill=3, max_ctx=400, max_q=300)
+    raise KeyError(name)
+
+
+SMALL = ["C1", "ragged-tiny", "ragged-g4-d128", "ragged-g8-d128", "ragged-g4-d256", "ragged-g1-d128", "edge-lens",
+         "decode-only", "prefill-only"]
+
+
+def test_device_generator_matches_host():
+    n = 1 << 16
+    for seed, tid, start in [(0, gen.TENSOR_Q, 0), (7, gen.TENSOR_K_POOL, 3_000_000_001), (203, gen.TENSOR_V_NEW, 12345)]:
+        t = torch.empty(n + 3, dtype=torch.bfloat16, device="cuda:0")
+        sdev.fill_bf16(t, seed, tid, start)
+        assert (sdev.bits(t) == gen.bf16_normal(seed, tid, start, n + 3)).all()
+
+
+@pytest.mark.parametrize("name", SMALL)
+def test_kv_append_and_gather_bit_exact(name):
+    batch = _small_case(name)
+    inp = helpers.host_inputs(batch)
+    d = gc.run_gpu(batch, inp)
+    _, kp, vp = gc.run_oracle(batch, inp, rows=np.zeros(0, dtype=np.int64))
+    assert (sdev.bits(d["k_pool"]) == kp).all(), "K pool differs from the oracle's after append"
+    assert (sdev.bits(d["v_pool"]) == vp).all(), "V pool differs from the oracle's after append"
+    osh = gc.oracle_shape(batch)
+    sh = batch.shape
+    for s in range(batch.n_seq):
+        kv = int(batch.kv_lens[s])
+        if kv == 0:
+            continue
+        k_out = torch.empty((kv, sh.num_kv_heads, sh.head_dim), dtype=torch.bfloat16, device="cuda:0")
+        v_out = torch.empty_like(k_out)
+        d["pa"].kv_gather(d["k_pool"], d["v_pool"], d["bt"][s], kv, k_out, v_out)
+        kg, vg = oracle.kv_gather(osh, kp, vp, batch.block_tables, s, kv)
+        assert (sdev.bits(k_out) == kg).all() and (sdev.bits(v_out) == vg).all()
+
+
+@pytest.mark.parametrize("name", SMALL)
+def test_attention_parity_small(name):
+    batch = _small_case(name)
+    inp = helpers.host_inputs(batch)
+    d = gc.run_gpu(batch, inp)
+    ref, _, _ = gc.run_oracle(batch, inp)
+    gc.check_close(sdev.bits(d["out"]), ref, name)
+
+
+@pytest.mark.parametrize("name", ["C1", "ragged-g4-d128", "ragged-g4-d256"])
+def test_debug_simple_kernel_parity(name):
+    batch = _small_case(name)
+    inp = helpers.host_inputs(batch)
+    d = gc.run_gpu(batch, inp, flags=binding.PA_FLAG_DEBUG_SIMPLE)
+    ref, _, _ = gc.run_oracle(batch, inp)
+    gc.check_close(sdev.bits(d["out"]), ref, name + "/simple")
+
+
+def test_split_kv_groups_merge_in_launch():
+    """Few long decode sequences: every (seq, head) group is cut into many items -> partials + last-arriver merge."""
+    W = workloads
+    batch = W.make_batch("split", W.GEMMA3_1B, 209, [1, 1, 1], [5000, 3333, 4097], 3)
+    inp = helpers.host_inputs(batch)
+    d = gc.run_gpu(batch, inp, repeat=3)          # repeat: counters must self-reset between launches
+    assert d["pa"].plan_info(2) > 3, "expected split items"
+    ref, _, _ = gc.run_oracle(batch, inp)
+    gc.check_close(sdev.bits(d["out"]), ref, "split")
+
+
+def test_repeated_launches_are_deterministic_and_reset_state():
+    batch = _small_case("ragged-g4-d128")
+    inp = helpers.host_inputs(batch)
+    d1 = gc.run_gpu(batch, inp, repeat=1)
+    d2 = gc.run_gpu(batch, inp, repeat=4)
+    assert (sdev.bits(d1["out"]) == sdev.bits(d2["out"])).all()
+
+
+@pytest.mark.parametrize("r", [0.0, 0.1, 0.5, 1.0])
+def test_config2_parity(r):
+    batch = workloads.config2(r)
+    d = gc.run_gpu(batch, None)
+    inp = dict(q=batch.q_bits(), k_new=batch.kv_new_bits()[0], v_new=batch.kv_new_bits()[1],
+               k_pool=sdev.bits(d["pool_before"][0]), v_pool=sdev.bits(d["pool_before"][1]))
+    # the device-filled pool must be the host stream (sampled), so the oracle's inputs are not the CUDA path's
+    idx = np.random.default_rng(1).integers(0, batch.pool_elems(), 4096)
+    valid = helpers.slot_valid_mask(batch, "ctx")
+    flat_valid = np.broadcast_to(valid[:, None, :, None], inp["k_pool"].shape).reshape(-1)[idx]
+    host = gen.bf16_normal_at(batch.seed, gen.TENSOR_K_POOL, idx.astype(np.uint64))
+    assert (inp["k_pool"].reshape(-1)[idx][flat_valid] == host[flat_valid]).all()
+    rng = np.random.default_rng(2)
+    rows = np.unique(np.concatenate([rng.integers(0, batch.n_tok, 96), [0, batch.n_tok - 1],
+                                     batch.cu_seqlens_q[:-1][-6:], batch.cu_seqlens_q[1:][-6:] - 1]))
+    ref, kp, vp = gc.run_oracle(batch, inp, rows=rows)
+    assert (sdev.bits(d["k_pool"]) == kp).all() and (sdev.bits(d["v_pool"]) == vp).all()
+    gc.check_close(sdev.bits(d["out"])[rows], ref, batch.name)
+
+
+def test_config3_full_size_sampled():
+    batch = workloads.config3()
+    d = gc.run_gpu(batch, None)
+    inp = dict(q=batch.q_bits(), k_new=batch.kv_new_bits()[0], v_new=batch.kv_new_bits()[1],
+               k_pool=sdev.bits(d["pool_before"][0]), v_pool=sdev.bits(d["pool_before"][1]))
+    rows = np.random.default_rng(3).choice(batch.n_tok, 48, replace=False)
+    ref, kp, vp = gc.run_oracle(batch, inp, rows=rows)
+    assert (sdev.bits(d["k_pool"]) == kp).all() and (sdev.bits(d["v_pool"]) == vp).all()
+    gc.check_close(sdev.bits(d["out"])[rows], ref, batch.name)
+    got = gen.bf16_to_f64(sdev.bits(d["out"]))
+    assert np.isfinite(got).all()                       # property at full size: no sentinel leaked anywhere
+
+
+def test_empty_and_degenerate_batches():
+    W = workloads
+    pa = binding.PagedAttention(8, 2, 128, 64, 8, 256, 8)
+    dev = "cuda:0"
+    z = torch.zeros(1, dtype=torch.int32, device=dev)
+    # n_seq = 0: every call is a no-op returning OK
+    pa.plan(np.zeros(1, np.int32), np.zeros(0, np.int32), 0, 0)
+    pa.kv_append(None, None, None, None, z, z, z, 0, 0)
+    q = torch.zeros((1, 8, 128), dtype=torch.bfloat16, device=dev)
+    pa.batch_attention(q, q, q, z, z, z, 0.1, q)
+    # q_len = 0 sequence inside the prefill range (R10)
+    batch = W.make_batch("zero-q", W.TINY, 210, [1, 0, 5, 0], [20, 40, 3, 0], 1, num_blocks=64, min_table_width=8)
+    inp = helpers.host_inputs(batch)
+    d = gc.run_gpu(batch, inp, pa=pa)
+    ref, _, _ = gc.run_oracle(batch, inp)
+    gc.check_close(sdev.bits(d["out"]), ref, "zero-q")
+
+
+def test_error_codes():
+    pa = binding.PagedAttention(8, 2, 128, 64, 4, 64, 8)
+    with pytest.raises(binding.PaError) as e:
+        pa.plan(np.array([0, 2, 3], np.int32), np.array([5, 5], np.int32), 2, 1)        # decode q_len = 2
+    assert e.value.code == binding.PA_ERR_INVALID
+    with pytest.raises(binding.PaError) as e:
+        pa.plan(np.array([0, 1, 0], np.int32), np.array([5, 5], np.int32), 2, 1)        # non-monotone
+    assert e.value.code == binding.PA_ERR_INVALID
+    with pytest.raises(binding.PaError) as e:
+        pa.plan(np.array([0, 1], np.int32), np.array([8 * 16], np.int32), 1, 1)         # kv_len > table width
+    assert e.value.code == binding.PA_ERR_INVALID
+    with pytest.raises(binding.PaError) as e:
+        pa.plan(np.arange(6, dtype=np.int32), np.zeros(5, np.int32), 5, 5)              # n_seq > max_seqs
+    assert e.value.code == binding.PA_ERR_INVALID
+    with pytest.raises(binding.PaError) as e:
+        pa.timer_fit(0.5)
+    assert e.value.code == binding.PA_ERR_TIMER
+    with pytest.raises(binding.PaError) as e:
+        binding.PagedAttention(8, 2, 64, 64, 4, 64, 8)
+    assert e.value.code == binding.PA_ERR_UNSUPPORTED
+    ws = pa.workspace
+    pa.workspace = ws[: 1024]
+    with pytest.raises(binding.PaError) as e:
+        pa.plan(np.array([0, 1], np.int32), np.array([3], np.int32), 1, 1)
+    assert e.value.code == binding.PA_ERR_WORKSPACE
+    pa.workspace = ws
+
+
+def test_timer_fit_matches_oracle_fit():
+    pa = binding.PagedAttention(8, 2, 128, 64, 4, 64, 8)
+    rng = np.random.default_rng(4)
+    ns, Ts = [], []
+    for n in (512, 1024, 2048, 4096):
+        reps = 3e-6 + 1.1e-8 * n + rng.normal(0, 2e-7, 7)
+        for t in reps:
+            pa.timer_record(0.3, n, float(abs(t)))
+        ns.append(n)
+        Ts.append(float(np.median(np.abs(reps))))
+    a, b, r2, npts = pa.timer_fit(0.3)
+    oa, ob, or2 = oracle.fit(ns, Ts)
+    assert npts == 4 and abs(a - oa) < 1e-15 and abs(b - ob) < 1e-18 and abs(r2 - or2) < 1e-12
+    pa.timer_begin()
+    sec = pa.timer_end(0.7, 128)
+    assert 0 <= sec < 1.0
