@@ -30,11 +30,14 @@ struct pa_ctx {
     // current plan
     bool planned = false;
     PlanView view{};
-    int32_t decode_ctas = 0, n_simple_tiles = 0, launches_per_call = 0, prefill_ctas = 0;
+    int32_t decode_ctas = 0, n_simple_tiles = 0, launches_per_call = 0, prefill_ctas = 0, p_in_tmem = 1;
+    int32_t planned_n_tok = 0;
     // tensor-map cache
     const void* tm_k_ptr = nullptr;
     const void* tm_v_ptr = nullptr;
-    CUtensorMap tmK{}, tmV{};
+    const void* tm_q_ptr = nullptr;
+    int32_t tm_q_ntok = -1;
+    CUtensorMap tmK{}, tmV{}, tmQ{};
     // timer
     cudaEvent_t t0 = nullptr, t1 = nullptr;
     std::map<int, std::map<int, std::vector<double>>> samples;  // r per-mille -> n_tok -> seconds
@@ -81,6 +84,22 @@ int32_t make_pool_map(pa_ctx* ctx, const void* pool, CUtensorMap* out) {
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(ctx, PA_ERR_CUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
+    return PA_OK;
+}
+
+// q[n_tok][Hq][D] bf16 -> 3-D tensor map, box = 64 columns x 1 head x 128 token rows, 128B swizzle
+// (rows past n_tok are zero-filled by the TMA unit)
+int32_t make_q_map(pa_ctx* ctx, const void* q, int32_t n_tok, CUtensorMap* out) {
+    const pa_config& c = ctx->cfg;
+    const cuuint64_t D = c.head_dim, Hq = c.num_q_heads;
+    cuuint64_t dims[3] = {D, Hq, (cuuint64_t)n_tok};
+    cuuint64_t strides[2] = {D * 2, Hq * D * 2};
+    cuuint32_t box[3] = {64, 1, (cuuint32_t)kQTile};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = g_encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(q), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(ctx, PA_ERR_CUDA, "cuTensorMapEncodeTiled(q) failed (" + std::to_string((int)r) + ")");
     return PA_OK;
 }
 
@@ -295,13 +314,24 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     int64_t off_t = off_b + align_up((int64_t)(n_bundles + 1) * 4, 256);
     PreTile* tiles = reinterpret_cast<PreTile*>(ctx->h_stage + off_t);
     int32_t n_tiles = 0;
+    double pre_flops = 0.0;
     for (int s = simple_all ? 0 : num_decode_seqs; s < n_seq; ++s) {
         const int32_t ql = h_cu[s + 1] - h_cu[s];
         for (int32_t q0 = 0; q0 < ql; q0 += kQTile) {
             if (n_tiles >= ctx->max_tiles) return fail(ctx, PA_ERR_INVALID, "pa_plan: tile list overflow");
-            tiles[n_tiles++] = PreTile{s, q0, std::min(kQTile, ql - q0), h_ctx[s]};
+            const int32_t rows = std::min(kQTile, ql - q0);
+            tiles[n_tiles++] = PreTile{s, q0, rows, h_ctx[s], h_ctx[s] + ql, h_cu[s], {0, 0}};
+            pre_flops += 4.0 * D * c.num_q_heads * rows * ((double)h_ctx[s] + q0 + 0.5 * rows);
         }
     }
+    // longest first: the queue then hands out units in LPT order (causal tiles late in a chunk see more keys)
+    std::stable_sort(tiles, tiles + n_tiles, [](const PreTile& a, const PreTile& b) {
+        return a.ctx + a.q_begin + a.q_rows > b.ctx + b.q_begin + b.q_rows;
+    });
+    const int prefill_mode = simple_all ? 2 : env_int("PA_PREFILL_MODE", 0);   // 0 P in TMEM, 1 P in smem, 2 plain kernel
+    const int NQ = D == 128 ? 2 : 1;
+    const int32_t head_groups = (G + NQ - 1) / NQ;
+    const int32_t n_units = prefill_mode == 2 ? 0 : n_tiles * Hkv * head_groups;
     const int64_t used = off_t + align_up((int64_t)n_tiles * sizeof(PreTile), 256);
 
     // ---- upload
@@ -325,10 +355,30 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     v.n_bundles = n_bundles;
     v.n_tiles = n_tiles;
     v.n_split = n_split;
-    ctx->decode_ctas = n_bundles > 0 ? std::min(ctx->num_sms, n_bundles) : 0;
-    ctx->n_simple_tiles = n_tiles;
-    ctx->prefill_ctas = 0;
-    ctx->launches_per_call = (ctx->decode_ctas > 0) + (n_tiles > 0);
+    v.n_units = n_units;
+    v.head_groups = head_groups;
+    // ---- CTA partition of the single launch (a7): share the SMs in proportion to the estimated
+    // tensor time of the prefill units and HBM time of the decode bundles; CTAs switch role when
+    // their own queue runs dry, so the split only has to be roughly right.
+    const int sms = ctx->num_sms;
+    int32_t pre_ctas = 0, dec_ctas = 0;
+    if (n_units > 0 && n_bundles > 0) {
+        const double t_pre = pre_flops / (0.45 * 1.4e15), t_dec = (double)total_blocks * kBlock * D * 2 * 2 / 6.5e12;
+        pre_ctas = (int32_t)std::lround(sms * t_pre / (t_pre + t_dec));
+        pre_ctas = env_int("PA_PREFILL_CTAS", pre_ctas);
+        pre_ctas = std::max(1, std::min({pre_ctas, sms - 1, n_units}));
+        dec_ctas = std::min(sms - pre_ctas, n_bundles);
+    } else if (n_units > 0) {
+        pre_ctas = std::min(sms, n_units);
+    } else if (n_bundles > 0) {
+        dec_ctas = std::min(sms, n_bundles);
+    }
+    ctx->decode_ctas = dec_ctas;
+    ctx->prefill_ctas = pre_ctas;
+    ctx->p_in_tmem = prefill_mode == 0;
+    ctx->n_simple_tiles = prefill_mode == 2 ? n_tiles : 0;
+    ctx->planned_n_tok = n_tok;
+    ctx->launches_per_call = (dec_ctas + pre_ctas > 0) + (ctx->n_simple_tiles > 0);
     ctx->planned = true;
     return PA_OK;
 }
@@ -352,6 +402,12 @@ int32_t pa_batch_attention(pa_ctx* ctx, const void* q, const void* k_pool, const
         if (rc != PA_OK) return rc;
         ctx->tm_v_ptr = v_pool;
     }
+    if (ctx->view.n_units > 0 && (ctx->tm_q_ptr != q || ctx->tm_q_ntok != ctx->planned_n_tok)) {
+        int32_t rc = make_q_map(ctx, q, ctx->planned_n_tok, &ctx->tmQ);
+        if (rc != PA_OK) return rc;
+        ctx->tm_q_ptr = q;
+        ctx->tm_q_ntok = ctx->planned_n_tok;
+    }
     AttnLaunch a;
     a.sh = LaunchShape{ctx->cfg.num_q_heads, ctx->cfg.num_kv_heads, ctx->cfg.head_dim, ctx->cfg.max_blocks_per_seq};
     a.q = q; a.out = out; a.k_pool = k_pool; a.v_pool = v_pool;
@@ -359,7 +415,10 @@ int32_t pa_batch_attention(pa_ctx* ctx, const void* q, const void* k_pool, const
     a.softmax_scale = softmax_scale;
     a.plan = ctx->view;
     a.decode_ctas = ctx->decode_ctas;
+    a.prefill_ctas = ctx->prefill_ctas;
+    a.p_in_tmem = ctx->p_in_tmem;
     a.n_simple_tiles = ctx->n_simple_tiles;
+    a.tmQ = ctx->view.n_units > 0 ? &ctx->tmQ : nullptr;
     a.tmK = &ctx->tmK; a.tmV = &ctx->tmV;
     int launches = 0;
     cudaError_t e = launch_attention(a, static_cast<cudaStream_t>(stream), &launches);

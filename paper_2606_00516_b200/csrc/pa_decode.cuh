@@ -30,8 +30,8 @@ struct AttnParams {
     int32_t Hq, Hkv, G;
     float scale_log2;             // softmax_scale * log2(e)
     PlanView plan;
-    int32_t decode_workers;       // total decode warps in the launch
-    int32_t decode_cta_begin;     // first CTA with the decode role (mixed launch)
+    int32_t decode_workers;       // decode warps with a statically assigned first bundle (= initial decode CTAs x 8)
+    int32_t prefill_ctas;         // CTAs [0, prefill_ctas) start in the prefill role (first unit = blockIdx.x)
 };
 
 template <int D>
@@ -42,16 +42,18 @@ struct DecodeCfg {
     static constexpr int kKSteps = D / 16;                // k-steps of QK^T == m-tiles of O^T
     static constexpr int kBoxes = D / 64;                 // 64-column TMA boxes per tile
     static constexpr int kFifo = 4;                       // opened-but-unfinished items per warp
-    static constexpr int kAuxBytes = 256;                 // per warp: kRing mbarriers (<= 48 B) + fifo (128 B)
+    static constexpr int kAuxBytes = 192;                 // per warp: kRing mbarriers (<= 48 B, at +0) + fifo (128 B, at +64)
     static constexpr int kWarpBytes = kRingBytes + kAuxBytes;
     static constexpr int kSmemBytes = kDecodeWarps * kRingBytes + kDecodeWarps * kAuxBytes + 1024;  // + align slack
 };
 
 // One persistent decode worker (a full warp).  ring: this warp's slot ring (1024-byte aligned);
-// aux: this warp's 256-byte scratch (mbarriers, item fifo).
+// aux: this warp's 192-byte scratch (mbarriers, item fifo).  first_bundle: the statically assigned first
+// bundle, or -1 for a worker that joins late (its CTA finished the prefill role) and takes every bundle
+// from the queue.
 template <int D>
 __device__ __forceinline__ void decode_worker(const AttnParams& p, const CUtensorMap* tmK, const CUtensorMap* tmV,
-                                              uint8_t* ring, uint8_t* aux, int worker_id) {
+                                              uint8_t* ring, uint8_t* aux, int first_bundle) {
     using Cfg = DecodeCfg<D>;
     constexpr int R = Cfg::kRing, UNIT = Cfg::kUnit, KS = Cfg::kKSteps, FQ = Cfg::kFifo;
     const int lane = lane_id(), g = lane >> 2, t = lane & 3;
@@ -73,8 +75,12 @@ __device__ __forceinline__ void decode_worker(const AttnParams& p, const CUtenso
     int iss_item = 0, iss_item_end = 0;
     bool iss_open = false, iss_isV = false, queue_done = false;
     int iss_seq = 0, iss_kvh = 0, iss_blk = 0, iss_blk_end = 0, iss_blkid = 0;
-    int next_bundle = worker_id, nb_l0 = 0;
+    int next_bundle = first_bundle, nb_l0 = 0;
     bool have_prefetched = false;
+    if (first_bundle < 0) {
+        if (lane == 0) nb_l0 = p.decode_workers + atomicAdd(&pl.queue[0], 1);
+        have_prefetched = true;
+    }
     int f_head = 0, f_tail = 0;
     // ---- consume cursor
     bool con_open = false, con_isV = false;
@@ -294,14 +300,6 @@ __device__ __forceinline__ void decode_worker(const AttnParams& p, const CUtenso
         ++u_con;
     }
 
-    // queue self-reset: the last worker to run dry zeroes the counters for the next launch
-    if (lane == 0) {
-        if (atomicAdd(&pl.queue[1], 1) == p.decode_workers - 1) {
-            pl.queue[0] = 0;
-            pl.queue[1] = 0;
-            __threadfence();
-        }
-    }
 }
 
 }  // namespace pa

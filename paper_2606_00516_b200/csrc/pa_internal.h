@@ -31,12 +31,15 @@ struct PreTile {
     int32_t q_begin;   // first query (within the chunk) of the tile
     int32_t q_rows;    // rows in the tile (<= kQTile)
     int32_t ctx;       // cached tokens before the chunk: query j sees keys 0 .. ctx + j
+    int32_t kv_len;    // ctx + q_len of the whole chunk (slots at positions >= kv_len hold nothing)
+    int32_t row0;      // cu_seqlens_q[seq]: first packed token row of the chunk
+    int32_t pad[2];
 };
-static_assert(sizeof(PreTile) == 16, "PreTile layout");
+static_assert(sizeof(PreTile) == 32, "PreTile layout");
 
 // Device-side view of the planned workspace (all pointers into the caller's workspace buffer).
 struct PlanView {
-    int32_t* queue;            // [0] next bundle, [1] finished workers, [2] next prefill unit, [3] finished prefill CTAs
+    int32_t* queue;            // [0] next decode bundle, [1] exited CTAs, [2] next prefill unit (all self-resetting)
     int32_t* group_counters;   // [num_decode_seqs * Hkv] arrivals of split groups (self-resetting)
     const DecItem* items;      // decode items in bundle order
     const int32_t* bundle_start; // [n_bundles + 1] item index ranges
@@ -44,6 +47,8 @@ struct PlanView {
     float2* part_ml;           // [slots][kMaxGroup] (m in log2 domain, l)
     float* part_o;             // [slots][G][D] unnormalised partial outputs
     int32_t n_items, n_bundles, n_tiles, n_split;
+    int32_t n_units;           // prefill work units = n_tiles * Hkv * head_groups (tcgen05 path; 0 = none)
+    int32_t head_groups;       // ceil(G / q-tiles per CTA): units per (tile, KV head)
 };
 
 }  // namespace pa

@@ -2,6 +2,7 @@
 #include "pa_launch.h"
 #include "pa_common.cuh"
 #include "pa_decode.cuh"
+#include "pa_prefill.cuh"
 #include "pa_simple.cuh"
 
 namespace pa {
@@ -105,33 +106,84 @@ cudaError_t launch_kv_gather(const LaunchShape& sh, const void* k_pool, const vo
     return cudaGetLastError();
 }
 
+
 // ------------------------------------------------------------------------------------------------
-// a5/a6 decode launch: persistent, one CTA per SM, kDecodeWarps independent workers per CTA.
+// a7 mixed single launch: one persistent CTA per SM, 12 warps.  CTAs [0, prefill_ctas) start in the
+// prefill role (tcgen05/TMEM), the rest in the decode role (8 TMA + mma.sync workers); when a CTA's
+// own queue runs dry it switches to the other role, so neither the tensor pipe nor HBM idles while
+// work remains.  The last CTA to leave resets the queues for the next launch.
+// Shared memory (from a 1024-byte aligned base): [0, 224 KB) tile region shared by the two roles,
+// then the prefill control block (256 B), then the decode workers' scratch (8 x 192 B).
 // ------------------------------------------------------------------------------------------------
-template <int D>
-__global__ void __launch_bounds__(kDecodeWarps * 32, 1)
-pa_decode_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV) {
+constexpr int kTileRegion = 224 * 1024;
+constexpr int kCtrlBytes = 256;
+constexpr int kAttnSmemBytes = 1024 + kTileRegion + kCtrlBytes + kDecodeWarps * 192;
+static_assert(kAttnSmemBytes <= 232448, "attention kernel shared memory");
+static_assert(kDecodeWarps * DecodeCfg<128>::kRingBytes <= kTileRegion, "decode rings fit the tile region");
+
+template <int D, bool kPinTmem>
+__global__ void __launch_bounds__(kAttnThreads, 1)
+pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+                    const __grid_constant__ CUtensorMap tmV) {
     extern __shared__ uint8_t smem_raw[];
-    uint8_t* base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    PrefillCtrl* ctrl = reinterpret_cast<PrefillCtrl*>(tiles + kTileRegion);
+    uint8_t* dec_aux = tiles + kTileRegion + kCtrlBytes;
     const int warp = threadIdx.x >> 5;
-    uint8_t* ring = base + warp * DecodeCfg<D>::kRingBytes;
-    uint8_t* aux = base + kDecodeWarps * DecodeCfg<D>::kRingBytes + warp * DecodeCfg<D>::kAuxBytes;
+    const PlanView& pl = p.plan;
     if (threadIdx.x == 0) {
         tma_prefetch_desc(&tmK);
         tma_prefetch_desc(&tmV);
+        if (pl.n_units > 0) {
+            tma_prefetch_desc(&tmQ);
+            prefill_init_barriers(ctrl);
+            fence_mbar_init();
+            fence_proxy_async();
+        }
     }
-    // interleave so that the first gridDim.x bundles land on distinct SMs
-    const int worker_id = warp * gridDim.x + blockIdx.x;
-    decode_worker<D>(p, &tmK, &tmV, ring, aux, worker_id);
+    __syncthreads();
+    const bool starts_prefill = (int)blockIdx.x < p.prefill_ctas;
+    const int dec_rank = (int)blockIdx.x - p.prefill_ctas;       // rank among the initial decode CTAs
+    const int dec_ctas = p.decode_workers / kDecodeWarps;
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {
+        const bool do_prefill = (pass == 0) == starts_prefill;
+        if (do_prefill) {
+            // late joiners only if units beyond the statically assigned ones exist
+            if (pl.n_units > 0 && (starts_prefill || pl.n_units > p.prefill_ctas))
+                prefill_role<D, kPinTmem>(p, &tmQ, &tmK, &tmV, tiles, ctrl, starts_prefill ? (int)blockIdx.x : -1);
+        } else {
+            if (pl.n_bundles > 0 && (!starts_prefill || pl.n_bundles > p.decode_workers) && warp < kDecodeWarps) {
+                // interleave so that the first dec_ctas bundles land on distinct SMs
+                const int first = starts_prefill ? -1 : warp * dec_ctas + dec_rank;
+                decode_worker<D>(p, &tmK, &tmV, tiles + warp * DecodeCfg<D>::kRingBytes, dec_aux + warp * DecodeCfg<D>::kAuxBytes,
+                                 first);
+            }
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        if (atomicAdd(&pl.queue[1], 1) == (int)gridDim.x - 1) {
+            pl.queue[0] = 0;
+            pl.queue[1] = 0;
+            pl.queue[2] = 0;
+            __threadfence();
+        }
+    }
 }
 
-int decode_smem_bytes(int D) { return D == 128 ? DecodeCfg<128>::kSmemBytes : DecodeCfg<256>::kSmemBytes; }
+int attention_smem_bytes() { return kAttnSmemBytes; }
+
+template <int D, bool T>
+static cudaError_t set_attr() {
+    return cudaFuncSetAttribute(pa_attention_kernel<D, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kAttnSmemBytes);
+}
 
 cudaError_t configure_kernels() {
-    cudaError_t e;
-    e = cudaFuncSetAttribute(pa_decode_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, DecodeCfg<128>::kSmemBytes);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(pa_decode_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, DecodeCfg<256>::kSmemBytes);
+    cudaError_t e = set_attr<128, true>();
+    if (e == cudaSuccess) e = set_attr<128, false>();
+    if (e == cudaSuccess) e = set_attr<256, true>();
+    if (e == cudaSuccess) e = set_attr<256, false>();
     return e;
 }
 
@@ -149,15 +201,20 @@ cudaError_t launch_attention(const AttnLaunch& a, cudaStream_t stream, int* laun
     p.scale_log2 = a.softmax_scale * 1.4426950408889634f;
     p.plan = a.plan;
     p.decode_workers = a.decode_ctas * kDecodeWarps;
-    p.decode_cta_begin = 0;
+    p.prefill_ctas = a.prefill_ctas;
     int launches = 0;
     cudaError_t e = cudaSuccess;
-    if (a.decode_ctas > 0 && a.plan.n_bundles > 0) {
-        dim3 grid(a.decode_ctas), block(kDecodeWarps * 32);
-        if (a.sh.D == 128)
-            pa_decode_kernel<128><<<grid, block, DecodeCfg<128>::kSmemBytes, stream>>>(p, *a.tmK, *a.tmV);
-        else
-            pa_decode_kernel<256><<<grid, block, DecodeCfg<256>::kSmemBytes, stream>>>(p, *a.tmK, *a.tmV);
+    const int grid_ctas = a.decode_ctas + a.prefill_ctas;
+    if (grid_ctas > 0) {
+        dim3 grid(grid_ctas), block(kAttnThreads);
+        const CUtensorMap& tq = a.tmQ ? *a.tmQ : *a.tmK;   // unused when there are no prefill units
+        if (a.sh.D == 128) {
+            if (a.p_in_tmem) pa_attention_kernel<128, true><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, *a.tmK, *a.tmV);
+            else pa_attention_kernel<128, false><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, *a.tmK, *a.tmV);
+        } else {
+            if (a.p_in_tmem) pa_attention_kernel<256, true><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, *a.tmK, *a.tmV);
+            else pa_attention_kernel<256, false><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, *a.tmK, *a.tmV);
+        }
         ++launches;
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;

@@ -31,8 +31,11 @@ struct AttnLaunch {
     const int32_t* block_tables;
     float softmax_scale;
     PlanView plan;
-    int32_t decode_ctas;     // CTAs with the decode role (0 = none)
-    int32_t n_simple_tiles;  // tiles routed to the plain kernel (v0 prefill / debug)
+    int32_t decode_ctas;     // CTAs that start in the decode role (0 = none)
+    int32_t prefill_ctas;    // CTAs that start in the prefill role (0 = none)
+    int32_t p_in_tmem;       // prefill variant: P staged in TMEM (1) or shared memory (0)
+    int32_t n_simple_tiles;  // tiles routed to the plain kernel (debug)
+    const CUtensorMap* tmQ;  // host copy of the query tensor map (null without prefill units)
     const CUtensorMap* tmK;  // host copies of the pool tensor maps
     const CUtensorMap* tmV;
 };
@@ -40,6 +43,6 @@ struct AttnLaunch {
 // Set opt-in shared memory sizes once per process/device.
 cudaError_t configure_kernels();
 cudaError_t launch_attention(const AttnLaunch& a, cudaStream_t stream, int* launches_out);
-int decode_smem_bytes(int D);
+int attention_smem_bytes();
 
 }  // namespace pa

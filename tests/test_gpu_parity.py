@@ -76,13 +76,15 @@ def test_kv_append_and_gather_bit_exact(name):
         assert (sdev.bits(k_out) == kg).all() and (sdev.bits(v_out) == vg).all()
 
 
+@pytest.mark.parametrize("mode", [0, 1])      # prefill variant: P staged in TMEM (default) / in shared memory
 @pytest.mark.parametrize("name", SMALL)
-def test_attention_parity_small(name):
+def test_attention_parity_small(name, mode, monkeypatch):
+    monkeypatch.setenv("PA_PREFILL_MODE", str(mode))
     batch = _small_case(name)
     inp = helpers.host_inputs(batch)
     d = gc.run_gpu(batch, inp)
     ref, _, _ = gc.run_oracle(batch, inp)
-    gc.check_close(sdev.bits(d["out"]), ref, name)
+    gc.check_close(sdev.bits(d["out"]), ref, f"{name}/mode{mode}")
 
 
 @pytest.mark.parametrize("name", ["C1", "ragged-g4-d128", "ragged-g4-d256"])
