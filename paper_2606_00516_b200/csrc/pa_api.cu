@@ -37,7 +37,9 @@ struct pa_ctx {
     const void* tm_v_ptr = nullptr;
     const void* tm_q_ptr = nullptr;
     int32_t tm_q_ntok = -1;
-    CUtensorMap tmK{}, tmV{}, tmQ{};
+    const void* tm_qd_ptr = nullptr;
+    int32_t tm_qd_ntok = -1;
+    CUtensorMap tmK{}, tmV{}, tmQ{}, tmQd{};
     // timer
     cudaEvent_t t0 = nullptr, t1 = nullptr;
     std::map<int, std::map<int, std::vector<double>>> samples;  // r per-mille -> n_tok -> seconds
@@ -100,6 +102,22 @@ int32_t make_q_map(pa_ctx* ctx, const void* q, int32_t n_tok, CUtensorMap* out) 
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(ctx, PA_ERR_CUDA, "cuTensorMapEncodeTiled(q) failed (" + std::to_string((int)r) + ")");
+    return PA_OK;
+}
+
+// q[n_tok][Hq][D] bf16 viewed as [n_tok*Hq][D] -> 2-D tensor map, box = 64 columns x G head rows (the q heads of
+// one KV head of one decode token are G consecutive rows), 128B swizzle
+int32_t make_qdec_map(pa_ctx* ctx, const void* q, int32_t n_tok, CUtensorMap* out) {
+    const pa_config& c = ctx->cfg;
+    const cuuint64_t D = c.head_dim;
+    cuuint64_t dims[2] = {D, (cuuint64_t)n_tok * c.num_q_heads};
+    cuuint64_t strides[1] = {D * 2};
+    cuuint32_t box[2] = {64, (cuuint32_t)ctx->G};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = g_encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(q), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(ctx, PA_ERR_CUDA, "cuTensorMapEncodeTiled(q decode) failed (" + std::to_string((int)r) + ")");
     return PA_OK;
 }
 
@@ -408,6 +426,12 @@ int32_t pa_batch_attention(pa_ctx* ctx, const void* q, const void* k_pool, const
         ctx->tm_q_ptr = q;
         ctx->tm_q_ntok = ctx->planned_n_tok;
     }
+    if (ctx->view.n_bundles > 0 && (ctx->tm_qd_ptr != q || ctx->tm_qd_ntok != ctx->planned_n_tok)) {
+        int32_t rc = make_qdec_map(ctx, q, ctx->planned_n_tok, &ctx->tmQd);
+        if (rc != PA_OK) return rc;
+        ctx->tm_qd_ptr = q;
+        ctx->tm_qd_ntok = ctx->planned_n_tok;
+    }
     AttnLaunch a;
     a.sh = LaunchShape{ctx->cfg.num_q_heads, ctx->cfg.num_kv_heads, ctx->cfg.head_dim, ctx->cfg.max_blocks_per_seq};
     a.q = q; a.out = out; a.k_pool = k_pool; a.v_pool = v_pool;
@@ -419,6 +443,7 @@ int32_t pa_batch_attention(pa_ctx* ctx, const void* q, const void* k_pool, const
     a.p_in_tmem = ctx->p_in_tmem;
     a.n_simple_tiles = ctx->n_simple_tiles;
     a.tmQ = ctx->view.n_units > 0 ? &ctx->tmQ : nullptr;
+    a.tmQd = ctx->view.n_bundles > 0 ? &ctx->tmQd : nullptr;
     a.tmK = &ctx->tmK; a.tmV = &ctx->tmV;
     int launches = 0;
     cudaError_t e = launch_attention(a, static_cast<cudaStream_t>(stream), &launches);

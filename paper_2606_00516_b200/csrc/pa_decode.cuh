@@ -1,17 +1,22 @@
 // a5 + a6: bandwidth-bound split-KV decode attention with in-launch flash-decoding merge.
 //
-// Design.  Every warp is an independent persistent worker that streams whole KV
-// blocks of (decode sequence, KV head) items through its own ring of shared-memory slots:
-//   * one elected lane issues TMA tensor loads (cp.async.bulk.tensor, 128B swizzle) of the 16-token
-//     K tile and V tile of each block, addressed through the block table, running up to kRing-1
-//     tiles ahead of the math — across item and bundle boundaries — so HBM requests never drain;
-//   * S^T = K·Q^T is computed with warp-level mma.sync m16n8k16 (M = 16 tokens of the block, N = the
-//     <= 8 q heads that share the KV head, K = head_dim), so K and V are read ONCE per KV head and the
-//     G = Hq/Hkv FMAs per loaded element run on the tensor pipe, not the fp32 lanes;
-//   * online softmax over tokens uses warp shuffles (xor 4, 8, 16); P^T is re-laid-out for the second
-//     MMA with movmatrix; O^T = V^T·P^T accumulates in registers;
-//   * an item that covers a whole (seq, head) writes its output row directly; split groups write
-//     (m, l, o) partials and the LAST arriving worker merges them (m = max m_i, l = Σ l_i 2^{m_i-m},
+// Design.  The decode role of a CTA runs 8 independent *streams*.  A stream is a
+// private ring of 4 KB shared-memory slots plus a 2-entry item fifo, filled by a producer lane and
+// drained by one consumer warp; streams never synchronise with each other, only producer <-> consumer
+// through mbarriers, so HBM requests of a stream keep flowing across item and bundle boundaries.
+//   producer (warps 0-3, two lanes each, one stream per lane): walks the planner's bundles of
+//     (decode sequence, KV head, block range) items; per item it copies the item descriptor into the
+//     fifo and fetches the G query rows of that KV head with one TMA box per 64 columns; per block it
+//     looks up the block table and issues TMA tensor loads (cp.async.bulk.tensor, 128B swizzle) of the
+//     16-token K tile and V tile.  All of this runs ahead of the math by the ring depth, so block-table
+//     and descriptor latencies are off the consumers' critical path;
+//   consumer (warps 4-11): S^T = K·Q^T with warp-level mma.sync m16n8k16 (M = 16 tokens of the block,
+//     N = the <= 8 q heads that share the KV head, K = head_dim), so K and V are read ONCE per KV head
+//     and the G = Hq/Hkv FMAs per loaded element run on the tensor pipe, not the fp32 lanes;
+//     online softmax over tokens with warp shuffles (xor 4, 8, 16); P^T re-laid-out for the second MMA
+//     with movmatrix; O^T = V^T·P^T accumulates in registers;
+//   an item that covers a whole (seq, head) writes its output rows directly; split groups write
+//     (m, l, o) partials and the LAST arriving consumer merges them (m = max m_i, l = Σ l_i 2^{m_i-m},
 //     o = Σ o_i 2^{m_i-m} / l) — one launch, no separate merge kernel.
 // HBM-bound: algorithmic bytes per decode token = kv_len·kvb + 2·qb + 4·ceil(kv_len/16).
 #pragma once
@@ -30,151 +35,176 @@ struct AttnParams {
     int32_t Hq, Hkv, G;
     float scale_log2;             // softmax_scale * log2(e)
     PlanView plan;
-    int32_t decode_workers;       // decode warps with a statically assigned first bundle (= initial decode CTAs x 8)
+    int32_t decode_workers;       // decode streams with a statically assigned first bundle (= initial decode CTAs x 8)
     int32_t prefill_ctas;         // CTAs [0, prefill_ctas) start in the prefill role (first unit = blockIdx.x)
 };
 
 template <int D>
 struct DecodeCfg {
-    static constexpr int kUnit = kBlock * D * 2;          // bytes of one K (or V) tile of one block-head
-    static constexpr int kRingBytes = 24576;              // per warp
-    static constexpr int kRing = kRingBytes / kUnit;      // 6 slots (D=128) / 3 slots (D=256)
-    static constexpr int kKSteps = D / 16;                // k-steps of QK^T == m-tiles of O^T
-    static constexpr int kBoxes = D / 64;                 // 64-column TMA boxes per tile
-    static constexpr int kFifo = 4;                       // opened-but-unfinished items per warp
-    static constexpr int kAuxBytes = 192;                 // per warp: kRing mbarriers (<= 48 B, at +0) + fifo (128 B, at +64)
-    static constexpr int kWarpBytes = kRingBytes + kAuxBytes;
-    static constexpr int kSmemBytes = kDecodeWarps * kRingBytes + kDecodeWarps * kAuxBytes + 1024;  // + align slack
+    static constexpr int kUnit = 4096;                    // ring slot: 16 tokens x 128 columns (two 64-column TMA boxes)
+    static constexpr int kHalves = D / 128;               // units per K (or V) tile of one block-head
+    static constexpr int kRing = (D == 128) ? 6 : 5;      // slots per stream
+    static constexpr int kFifo = 2;                       // items in flight per stream (descriptor + Q rows)
+    static constexpr int kQSlot = (D / 64) * 1024;        // Q rows of one item: D/64 boxes of 8 rows x 128 B
+    static constexpr int kStreamBytes = kRing * kUnit + kFifo * kQSlot;   // 28 KB
+    // per-stream scratch: full[kRing], empty[kRing], ffull[kFifo], fempty[kFifo] mbarriers, then the descriptors
+    static constexpr int kOffEmpty = 8 * kRing, kOffFFull = 16 * kRing, kOffFEmpty = 16 * kRing + 8 * kFifo;
+    static constexpr int kOffDesc = 128;
+    static constexpr int kAuxBytes = 192;
+    static_assert(kOffFEmpty + 8 * kFifo <= kOffDesc && kOffDesc + kFifo * 32 <= kAuxBytes, "decode scratch layout");
+    static_assert(kStreamBytes == 28 * 1024, "decode stream bytes");
 };
+constexpr int kDecodeProducerWarps = 4;                              // warps 0-3
+constexpr int kStreamsPerProducer = kDecodeWarps / kDecodeProducerWarps;
 
-// One persistent decode worker (a full warp).  ring: this warp's slot ring (1024-byte aligned);
-// aux: this warp's 192-byte scratch (mbarriers, item fifo).  first_bundle: the statically assigned first
-// bundle, or -1 for a worker that joins late (its CTA finished the prefill role) and takes every bundle
-// from the queue.
+// one thread, once per CTA, before the roles start
 template <int D>
-__device__ __forceinline__ void decode_worker(const AttnParams& p, const CUtensorMap* tmK, const CUtensorMap* tmV,
-                                              uint8_t* ring, uint8_t* aux, int first_bundle) {
+__device__ __forceinline__ void decode_init_barriers(uint8_t* dec_aux) {
     using Cfg = DecodeCfg<D>;
-    constexpr int R = Cfg::kRing, UNIT = Cfg::kUnit, KS = Cfg::kKSteps, FQ = Cfg::kFifo;
-    const int lane = lane_id(), g = lane >> 2, t = lane & 3;
-    const uint32_t ring_u32 = smem_u32(ring);
-    const uint32_t bar_u32 = smem_u32(aux);                       // kRing x 8 bytes
-    DecItem* fifo = reinterpret_cast<DecItem*>(aux + 64);         // FQ x 32 bytes
+    for (int s = 0; s < kDecodeWarps; ++s) {
+        const uint32_t a = smem_u32(dec_aux + s * Cfg::kAuxBytes);
+        for (int i = 0; i < 2 * Cfg::kRing + 2 * Cfg::kFifo; ++i) mbar_init(a + 8 * i, 1);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Producer lane of one stream.  first_bundle: the statically assigned first bundle, or -1 for a stream
+// that joins late (its CTA finished the prefill role) and takes every bundle from the queue.
+// ------------------------------------------------------------------------------------------------
+template <int D>
+__device__ __forceinline__ void decode_producer(const AttnParams& p, const CUtensorMap* tmQd, const CUtensorMap* tmK,
+                                                const CUtensorMap* tmV, uint8_t* stream_mem, uint8_t* aux,
+                                                int first_bundle) {
+    using Cfg = DecodeCfg<D>;
+    constexpr int R = Cfg::kRing, FQ = Cfg::kFifo, H = Cfg::kHalves;
     const PlanView& pl = p.plan;
-    const int G = p.G;
+    const uint32_t ring_u32 = smem_u32(stream_mem);
+    const uint32_t q_u32 = ring_u32 + R * Cfg::kUnit;
+    const uint32_t bar = smem_u32(aux);
+    const uint32_t q_bytes = (uint32_t)p.G * D * 2;
+    const uint64_t pol = policy_evict_first();
 
-    if (lane == 0) {
-        for (int i = 0; i < R; ++i) mbar_init(bar_u32 + 8 * i, 1);
-        fence_mbar_init();
-        fence_proxy_async();
-    }
-    __syncwarp();
-
-    uint32_t u_iss = 0, u_con = 0;
-    // ---- issue cursor (warp-uniform except iss_blkid / nb_l0 which live in lane 0)
-    int iss_item = 0, iss_item_end = 0;
-    bool iss_open = false, iss_isV = false, queue_done = false;
-    int iss_seq = 0, iss_kvh = 0, iss_blk = 0, iss_blk_end = 0, iss_blkid = 0;
-    int next_bundle = first_bundle, nb_l0 = 0;
-    bool have_prefetched = false;
-    if (first_bundle < 0) {
-        if (lane == 0) nb_l0 = p.decode_workers + atomicAdd(&pl.queue[0], 1);
-        have_prefetched = true;
-    }
-    int f_head = 0, f_tail = 0;
-    // ---- consume cursor
-    bool con_open = false, con_isV = false;
-    DecItem ci = {};
-    int con_blk = 0, nvalid = 16, q_row = 0, h0 = 0;
-    float m0 = 0.f, m1 = 0.f, l0 = 0.f, l1 = 0.f;
-    float o[KS][4];
-    uint32_t qf[KS][2];
-    uint32_t pb0 = 0, pb1 = 0;
-
+    uint32_t u_iss = 0, i_iss = 0;
+    int next_bundle = first_bundle;
+    if (next_bundle < 0) next_bundle = p.decode_workers + atomicAdd(&pl.queue[0], 1);
+    int item = 0, item_end = 0;
     for (;;) {
-        // =============================== issue side: keep the ring full
-        while (u_iss - u_con < (uint32_t)R) {
-            if (!iss_open) {
-                if (iss_item >= iss_item_end) {
-                    if (queue_done) break;
-                    if (have_prefetched) next_bundle = __shfl_sync(0xffffffffu, nb_l0, 0);
-                    if (next_bundle >= pl.n_bundles) { queue_done = true; break; }
-                    iss_item = pl.bundle_start[next_bundle];
-                    iss_item_end = pl.bundle_start[next_bundle + 1];
-                    if (lane == 0) nb_l0 = p.decode_workers + atomicAdd(&pl.queue[0], 1);  // consumed at the next bundle
-                    have_prefetched = true;
-                }
-                if (f_tail - f_head >= FQ) break;
-                const int4* src = reinterpret_cast<const int4*>(pl.items + iss_item);
-                int4 a = __ldg(src), b = __ldg(src + 1);
-                if (lane == 0) {
-                    int4* dst = reinterpret_cast<int4*>(fifo + (f_tail % FQ));
-                    dst[0] = a;
-                    dst[1] = b;
-                }
-                ++f_tail;
-                ++iss_item;
-                iss_seq = a.x; iss_kvh = a.y; iss_blk = a.z; iss_blk_end = a.w;
-                iss_open = true; iss_isV = false;
-            }
-            if (lane == 0) {
-                if (!iss_isV) iss_blkid = __ldg(p.block_tables + (int64_t)iss_seq * p.max_blocks_per_seq + iss_blk);
-                const uint32_t slot = u_iss % R;
-                const uint32_t bar = bar_u32 + 8 * slot, dst = ring_u32 + slot * UNIT;
-                mbar_expect_tx(bar, UNIT);
-                const CUtensorMap* tm = iss_isV ? tmV : tmK;
-#pragma unroll
-                for (int qd = 0; qd < Cfg::kBoxes; ++qd) tma_load_4d(dst + qd * 2048, tm, bar, qd * 64, 0, iss_kvh, iss_blkid);
-            }
-            ++u_iss;
-            if (iss_isV) {
-                ++iss_blk;
-                if (iss_blk == iss_blk_end) iss_open = false;
-            }
-            iss_isV = !iss_isV;
-        }
-        if (u_con == u_iss) {
-            if (queue_done) break;
+        if (item >= item_end) {
+            if (next_bundle >= pl.n_bundles) break;
+            item = __ldg(pl.bundle_start + next_bundle);
+            item_end = __ldg(pl.bundle_start + next_bundle + 1);
+            next_bundle = p.decode_workers + atomicAdd(&pl.queue[0], 1);   // result is needed one bundle later
             continue;
         }
-
-        // =============================== consume side: one tile per iteration
-        const uint32_t slot = u_con % R, parity = (u_con / R) & 1u;
-        const uint32_t tile = ring_u32 + slot * UNIT;
-        if (!con_open) {
-            __syncwarp();
-            ci = fifo[f_head % FQ];
-            con_blk = ci.blk_begin;
-            con_isV = false;
-            q_row = __ldg(p.cu_seqlens_q + ci.seq);
-            h0 = ci.kv_head * G;
-            const uint32_t* qp = reinterpret_cast<const uint32_t*>(p.q + ((int64_t)q_row * p.Hq + h0 + g) * D) + t;
+        // ---- open the item: descriptor + Q rows into the fifo entry
+        const int4* src = reinterpret_cast<const int4*>(pl.items + item);
+        const int4 a = __ldg(src), b = __ldg(src + 1);
+        ++item;
+        const int seq = a.x, kvh = a.y, blk_end = a.w;
+        int blk = a.z;
+        const int32_t* bt = p.block_tables + (int64_t)seq * p.max_blocks_per_seq;
+        int blkid = __ldg(bt + blk);
+        {
+            const uint32_t fs = i_iss % FQ;
+            mbar_wait(bar + Cfg::kOffFEmpty + 8 * fs, ((i_iss / FQ) & 1u) ^ 1u);
+            const uint32_t d = smem_u32(aux + Cfg::kOffDesc + 32 * fs);
+            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(d), "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w) : "memory");
+            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(d + 16), "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w) : "memory");
+            const uint32_t ff = bar + Cfg::kOffFFull + 8 * fs;
+            mbar_expect_tx(ff, q_bytes);
+            // decode sequences come first with q_len == 1 (R11), so the packed query row of sequence s is s
+            const int qrow = seq * p.Hq + kvh * p.G;
 #pragma unroll
-            for (int ks = 0; ks < KS; ++ks) {
-                qf[ks][0] = (g < G) ? __ldg(qp + ks * 8) : 0u;      // d = 16ks + 2t, +1
-                qf[ks][1] = (g < G) ? __ldg(qp + ks * 8 + 4) : 0u;  // d = 16ks + 8 + 2t, +1
-            }
-            m0 = m1 = -INFINITY;
-            l0 = l1 = 0.f;
-#pragma unroll
-            for (int i = 0; i < KS; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
-            con_open = true;
+            for (int c = 0; c < D / 64; ++c) tma_load_2d(q_u32 + fs * Cfg::kQSlot + c * 1024, tmQd, ff, c * 64, qrow);
+            ++i_iss;
         }
-        mbar_wait(bar_u32 + 8 * slot, parity);
-
-        if (!con_isV) {
-            // ---- S^T[16 tok x 8 heads] = K[16 x D] · Q^T[D x 8]
-            nvalid = min(16, ci.kv_len - con_blk * kBlock);
-            float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb[4] = {0.f, 0.f, 0.f, 0.f};
-            const uint32_t mi = lane >> 3, r8 = lane & 7;
-            const uint32_t row = r8 + 8 * (mi & 1);
+        // ---- stream the K and V tiles of the item's blocks
+        while (blk < blk_end) {
+            const int cur = blkid;
+            ++blk;
+            if (blk < blk_end) blkid = __ldg(bt + blk);   // prefetch the next block id behind this block's issue
 #pragma unroll
-            for (int ks = 0; ks < KS; ++ks) {
-                const uint32_t chunk = 2 * ks + (mi >> 1);          // 16-byte chunk along d
-                uint32_t a[4];
-                ldmatrix_x4(a, tile + (chunk >> 3) * 2048 + swz128(row, chunk & 7));
-                if (ks & 1) mma_bf16_16816(sb, a, qf[ks][0], qf[ks][1]);
-                else        mma_bf16_16816(sa, a, qf[ks][0], qf[ks][1]);
+            for (int isV = 0; isV < 2; ++isV) {
+#pragma unroll
+                for (int h = 0; h < H; ++h) {
+                    const uint32_t slot = u_iss % R;
+                    mbar_wait(bar + Cfg::kOffEmpty + 8 * slot, ((u_iss / R) & 1u) ^ 1u);
+                    const uint32_t full = bar + 8 * slot, dst = ring_u32 + slot * Cfg::kUnit;
+                    mbar_expect_tx(full, Cfg::kUnit);
+                    tma_load_4d_hint(dst, isV ? tmV : tmK, full, h * 128, 0, kvh, cur, pol);
+                    tma_load_4d_hint(dst + 2048, isV ? tmV : tmK, full, h * 128 + 64, 0, kvh, cur, pol);
+                    ++u_iss;
+                }
+            }
+        }
+    }
+    // ---- sentinel item: tells the consumer that the stream is finished
+    {
+        const uint32_t fs = i_iss % FQ;
+        mbar_wait(bar + Cfg::kOffFEmpty + 8 * fs, ((i_iss / FQ) & 1u) ^ 1u);
+        const uint32_t d = smem_u32(aux + Cfg::kOffDesc + 32 * fs);
+        asm volatile("st.shared.b32 [%0], %1;" ::"r"(d), "r"(-1) : "memory");
+        mbar_arrive(bar + Cfg::kOffFFull + 8 * fs);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Consumer warp of one stream.
+// ------------------------------------------------------------------------------------------------
+template <int D>
+__device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* stream_mem, uint8_t* aux) {
+    using Cfg = DecodeCfg<D>;
+    constexpr int R = Cfg::kRing, FQ = Cfg::kFifo, H = Cfg::kHalves, KS = D / 16;
+    const int lane = lane_id(), g = lane >> 2, t = lane & 3;
+    const uint32_t ring_u32 = smem_u32(stream_mem);
+    const uint32_t q_u32 = ring_u32 + R * Cfg::kUnit;
+    const uint32_t bar = smem_u32(aux);
+    const PlanView& pl = p.plan;
+    const int G = p.G;
+    const uint32_t mi = lane >> 3, r8 = lane & 7;
+
+    uint32_t u_con = 0, i_con = 0;
+    for (;;) {
+        const uint32_t fs = i_con % FQ;
+        mbar_wait(bar + Cfg::kOffFFull + 8 * fs, (i_con / FQ) & 1u);
+        const DecItem ci = *reinterpret_cast<const DecItem*>(aux + Cfg::kOffDesc + 32 * fs);
+        if (ci.seq < 0) break;
+        const uint32_t qs = q_u32 + fs * Cfg::kQSlot;
+        const int q_row = ci.seq, h0 = ci.kv_head * G;
+        float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+        float o[KS][4];
+#pragma unroll
+        for (int i = 0; i < KS; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
+
+        for (int blk = ci.blk_begin; blk < ci.blk_end; ++blk) {
+            const int nvalid = min(16, ci.kv_len - blk * kBlock);
+            // ---- S^T[16 tok x 8 heads] = K[16 x D] · Q^T[D x 8]
+            float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+            for (int h = 0; h < H; ++h) {
+                const uint32_t slot = u_con % R;
+                mbar_wait(bar + 8 * slot, (u_con / R) & 1u);
+                const uint32_t tile = ring_u32 + slot * Cfg::kUnit;
+                const uint32_t row = r8 + 8 * (mi & 1);
+#pragma unroll
+                for (int k2 = 0; k2 < 4; ++k2) {     // pairs of k-steps within the 128-column unit
+                    uint32_t qf[4];
+                    {   // B fragments of k-steps 2k2, 2k2+1: matrices = 16-byte chunks 4k2 + mi of the q rows
+                        const uint32_t cq = h * 16 + 4 * k2 + mi;
+                        ldmatrix_x4(qf, qs + (cq >> 3) * 1024 + swz128(r8, cq & 7));
+                    }
+#pragma unroll
+                    for (int kk = 0; kk < 2; ++kk) {
+                        const uint32_t chunk = 2 * (2 * k2 + kk) + (mi >> 1);     // 16-byte chunk along d within the unit
+                        uint32_t a[4];
+                        ldmatrix_x4(a, tile + (chunk >> 3) * 2048 + swz128(row, chunk & 7));
+                        if (kk) mma_bf16_16816(sb, a, qf[2], qf[3]);
+                        else    mma_bf16_16816(sa, a, qf[0], qf[1]);
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar + Cfg::kOffEmpty + 8 * slot);
+                ++u_con;
             }
             // thread holds tokens g (s0,s1) and g+8 (s2,s3) for heads 2t (s0,s2) and 2t+1 (s1,s3)
             float s0 = (sa[0] + sb[0]) * p.scale_log2, s1 = (sa[1] + sb[1]) * p.scale_log2;
@@ -197,109 +227,132 @@ __device__ __forceinline__ void decode_worker(const AttnParams& p, const CUtenso
 #pragma unroll
             for (int i = 0; i < KS; ++i) { o[i][0] *= c0; o[i][1] *= c1; o[i][2] *= c0; o[i][3] *= c1; }
             // P^T as the B operand of the second MMA (k = token, n = head): transpose the two 8x8 tiles
-            pb0 = movmatrix_trans(pack_bf16x2(p0, p1));
-            pb1 = movmatrix_trans(pack_bf16x2(p2, p3));
-            con_isV = true;
-        } else {
+            const uint32_t pb0 = movmatrix_trans(pack_bf16x2(p0, p1));
+            const uint32_t pb1 = movmatrix_trans(pack_bf16x2(p2, p3));
             // ---- O^T[D x 8 heads] += V^T[D x 16 tok] · P^T[16 tok x 8]
-            if (nvalid < 16) {   // last, partly filled block: unused V rows may hold anything (NaN): zero them
-                const int nz = (16 - nvalid) * 8;                    // 16-byte chunks per 64-column box
 #pragma unroll
-                for (int qd = 0; qd < Cfg::kBoxes; ++qd)
-                    for (int idx = lane; idx < nz; idx += 32)
-                        asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(tile + qd * 2048 + nvalid * 128 + idx * 16), "r"(0u) : "memory");
-                __syncwarp();
-            }
-            const uint32_t mi = lane >> 3, r8 = lane & 7;
-            const uint32_t row = r8 + 8 * (mi >> 1);               // token
+            for (int h = 0; h < H; ++h) {
+                const uint32_t slot = u_con % R;
+                mbar_wait(bar + 8 * slot, (u_con / R) & 1u);
+                const uint32_t tile = ring_u32 + slot * Cfg::kUnit;
+                if (nvalid < 16) {   // last, partly filled block: unused V rows may hold anything (NaN): zero them
+                    const int nz = (16 - nvalid) * 8;                    // 16-byte chunks per 64-column box
 #pragma unroll
-            for (int i = 0; i < KS; ++i) {
-                const uint32_t chunk = 2 * i + (mi & 1);
-                uint32_t a[4];
-                ldmatrix_x4_trans(a, tile + (chunk >> 3) * 2048 + swz128(row, chunk & 7));
-                mma_bf16_16816(o[i], a, pb0, pb1);
-            }
-            con_isV = false;
-            ++con_blk;
-            if (con_blk == ci.blk_end) {
-                // ---------------- item finished
-#pragma unroll
-                for (int off = 4; off <= 16; off <<= 1) {
-                    l0 += __shfl_xor_sync(0xffffffffu, l0, off);
-                    l1 += __shfl_xor_sync(0xffffffffu, l1, off);
-                }
-                const int ha = 2 * t, hb = 2 * t + 1;
-                if (ci.n_parts == 1) {
-                    const float i0 = 1.f / l0, i1 = 1.f / l1;
-                    __nv_bfloat16* oa = p.out + ((int64_t)q_row * p.Hq + h0 + ha) * D + g;
-                    __nv_bfloat16* ob = oa + D;
-#pragma unroll
-                    for (int i = 0; i < KS; ++i) {
-                        if (ha < G) { oa[16 * i] = __float2bfloat16_rn(o[i][0] * i0); oa[16 * i + 8] = __float2bfloat16_rn(o[i][2] * i0); }
-                        if (hb < G) { ob[16 * i] = __float2bfloat16_rn(o[i][1] * i1); ob[16 * i + 8] = __float2bfloat16_rn(o[i][3] * i1); }
-                    }
-                } else {
-                    const int ps = ci.part_base + ci.part_idx;
-                    if (g == 0) {
-                        if (ha < G) pl.part_ml[ps * kMaxGroup + ha] = make_float2(m0, l0);
-                        if (hb < G) pl.part_ml[ps * kMaxGroup + hb] = make_float2(m1, l1);
-                    }
-                    float* pa_ = pl.part_o + ((int64_t)ps * G + ha) * D + g;
-                    float* pb_ = pa_ + D;
-#pragma unroll
-                    for (int i = 0; i < KS; ++i) {
-                        if (ha < G) { pa_[16 * i] = o[i][0]; pa_[16 * i + 8] = o[i][2]; }
-                        if (hb < G) { pb_[16 * i] = o[i][1]; pb_[16 * i + 8] = o[i][3]; }
-                    }
-                    __threadfence();
+                    for (int qd = 0; qd < 2; ++qd)
+                        for (int idx = lane; idx < nz; idx += 32)
+                            asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(tile + qd * 2048 + nvalid * 128 + idx * 16), "r"(0u) : "memory");
                     __syncwarp();
-                    int last = 0;
-                    int32_t* ctr = pl.group_counters + ci.seq * p.Hkv + ci.kv_head;
-                    if (lane == 0) last = (atomicAdd(ctr, 1) == ci.n_parts - 1);
-                    last = __shfl_sync(0xffffffffu, last, 0);
-                    if (last) {
-                        // ---------------- a6 merge by the last-arriving worker
-                        __threadfence();
-                        constexpr int VPL = D / 32;                  // floats per lane
-                        for (int hh = 0; hh < G; ++hh) {
-                            float M = -INFINITY;
-                            for (int i = 0; i < ci.n_parts; ++i)
-                                M = fmaxf(M, __ldcg(&pl.part_ml[(ci.part_base + i) * kMaxGroup + hh]).x);
-                            float L = 0.f, acc[VPL];
-#pragma unroll
-                            for (int k = 0; k < VPL; ++k) acc[k] = 0.f;
-                            for (int i = 0; i < ci.n_parts; ++i) {
-                                const float2 ml = __ldcg(&pl.part_ml[(ci.part_base + i) * kMaxGroup + hh]);
-                                const float w = fast_exp2(ml.x - M);
-                                L += ml.y * w;
-                                const float4* src = reinterpret_cast<const float4*>(
-                                    pl.part_o + ((int64_t)(ci.part_base + i) * G + hh) * D + lane * VPL);
-#pragma unroll
-                                for (int k = 0; k < VPL / 4; ++k) {
-                                    const float4 v = __ldcg(src + k);
-                                    acc[4 * k] += w * v.x; acc[4 * k + 1] += w * v.y;
-                                    acc[4 * k + 2] += w * v.z; acc[4 * k + 3] += w * v.w;
-                                }
-                            }
-                            const float inv = 1.f / L;
-                            uint32_t packed[VPL / 2];
-#pragma unroll
-                            for (int k = 0; k < VPL / 2; ++k) packed[k] = pack_bf16x2(acc[2 * k] * inv, acc[2 * k + 1] * inv);
-                            uint32_t* dst = reinterpret_cast<uint32_t*>(p.out + ((int64_t)q_row * p.Hq + h0 + hh) * D + lane * VPL);
-                            if constexpr (VPL == 4) *reinterpret_cast<uint2*>(dst) = make_uint2(packed[0], packed[1]);
-                            else *reinterpret_cast<uint4*>(dst) = make_uint4(packed[0], packed[1], packed[2], packed[3]);
-                        }
-                        if (lane == 0) *ctr = 0;                      // self-reset for the next launch
-                    }
                 }
-                con_open = false;
-                ++f_head;
+                const uint32_t row = r8 + 8 * (mi >> 1);               // token
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const uint32_t chunk = 2 * i + (mi & 1);
+                    uint32_t a[4];
+                    ldmatrix_x4_trans(a, tile + (chunk >> 3) * 2048 + swz128(row, chunk & 7));
+                    mma_bf16_16816(o[h * 8 + i], a, pb0, pb1);
+                }
+                if (nvalid < 16) fence_proxy_async();   // generic-proxy zero fill before the slot's next TMA write
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar + Cfg::kOffEmpty + 8 * slot);
+                ++u_con;
             }
         }
-        __syncwarp();   // every lane is done with this slot before lane 0 re-arms it
-        ++u_con;
+        // ---------------- item finished
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar + Cfg::kOffFEmpty + 8 * fs);    // Q rows and descriptor are no longer needed
+        ++i_con;
+#pragma unroll
+        for (int off = 4; off <= 16; off <<= 1) {
+            l0 += __shfl_xor_sync(0xffffffffu, l0, off);
+            l1 += __shfl_xor_sync(0xffffffffu, l1, off);
+        }
+        const int ha = 2 * t, hb = 2 * t + 1;
+        if (ci.n_parts == 1) {
+            // O^T fragments -> (head = g, d = 16i + 2t, +1) via movmatrix: 4-byte stores, 16 B contiguous per head
+            const float i0 = 1.f / l0, i1 = 1.f / l1;
+            uint32_t* dst = reinterpret_cast<uint32_t*>(p.out + ((int64_t)q_row * p.Hq + h0 + g) * D) + t;
+#pragma unroll
+            for (int i = 0; i < KS; ++i) {
+                const uint32_t y0 = movmatrix_trans(pack_bf16x2(o[i][0] * i0, o[i][1] * i1));
+                const uint32_t y1 = movmatrix_trans(pack_bf16x2(o[i][2] * i0, o[i][3] * i1));
+                if (g < G) { dst[8 * i] = y0; dst[8 * i + 4] = y1; }
+            }
+        } else {
+            const int ps = ci.part_base + ci.part_idx;
+            if (g == 0) {
+                if (ha < G) pl.part_ml[ps * kMaxGroup + ha] = make_float2(m0, l0);
+                if (hb < G) pl.part_ml[ps * kMaxGroup + hb] = make_float2(m1, l1);
+            }
+            float* pa_ = pl.part_o + ((int64_t)ps * G + ha) * D + g;
+            float* pb_ = pa_ + D;
+#pragma unroll
+            for (int i = 0; i < KS; ++i) {
+                if (ha < G) { pa_[16 * i] = o[i][0]; pa_[16 * i + 8] = o[i][2]; }
+                if (hb < G) { pb_[16 * i] = o[i][1]; pb_[16 * i + 8] = o[i][3]; }
+            }
+            __threadfence();
+            __syncwarp();
+            int last = 0;
+            int32_t* ctr = pl.group_counters + ci.seq * p.Hkv + ci.kv_head;
+            if (lane == 0) last = (atomicAdd(ctr, 1) == ci.n_parts - 1);
+            last = __shfl_sync(0xffffffffu, last, 0);
+            if (last) {
+                // ---------------- a6 merge by the last-arriving consumer
+                __threadfence();
+                constexpr int VPL = D / 32;                  // floats per lane
+                for (int hh = 0; hh < G; ++hh) {
+                    float M = -INFINITY;
+                    for (int i = 0; i < ci.n_parts; ++i)
+                        M = fmaxf(M, __ldcg(&pl.part_ml[(ci.part_base + i) * kMaxGroup + hh]).x);
+                    float L = 0.f, acc[VPL];
+#pragma unroll
+                    for (int k = 0; k < VPL; ++k) acc[k] = 0.f;
+                    for (int i = 0; i < ci.n_parts; ++i) {
+                        const float2 ml = __ldcg(&pl.part_ml[(ci.part_base + i) * kMaxGroup + hh]);
+                        const float w = fast_exp2(ml.x - M);
+                        L += ml.y * w;
+                        const float4* src = reinterpret_cast<const float4*>(
+                            pl.part_o + ((int64_t)(ci.part_base + i) * G + hh) * D + lane * VPL);
+#pragma unroll
+                        for (int k = 0; k < VPL / 4; ++k) {
+                            const float4 v = __ldcg(src + k);
+                            acc[4 * k] += w * v.x; acc[4 * k + 1] += w * v.y;
+                            acc[4 * k + 2] += w * v.z; acc[4 * k + 3] += w * v.w;
+                        }
+                    }
+                    const float inv = 1.f / L;
+                    uint32_t packed[VPL / 2];
+#pragma unroll
+                    for (int k = 0; k < VPL / 2; ++k) packed[k] = pack_bf16x2(acc[2 * k] * inv, acc[2 * k + 1] * inv);
+                    uint32_t* dst = reinterpret_cast<uint32_t*>(p.out + ((int64_t)q_row * p.Hq + h0 + hh) * D + lane * VPL);
+                    if constexpr (VPL == 4) *reinterpret_cast<uint2*>(dst) = make_uint2(packed[0], packed[1]);
+                    else *reinterpret_cast<uint4*>(dst) = make_uint4(packed[0], packed[1], packed[2], packed[3]);
+                }
+                if (lane == 0) *ctr = 0;                      // self-reset for the next launch
+            }
+        }
     }
+}
 
+// The decode role of one CTA (12 warps): warps 0-3 produce (lanes 0,1 -> streams 2w, 2w+1), warps 4-11 consume.
+// dec_rank >= 0: rank among the CTAs that START in the decode role (static first bundles, interleaved so that
+// the first bundles land on distinct SMs); dec_rank < 0: late joiner, every bundle comes from the queue.
+template <int D>
+__device__ __forceinline__ void decode_role(const AttnParams& p, const CUtensorMap* tmQd, const CUtensorMap* tmK,
+                                            const CUtensorMap* tmV, uint8_t* tiles, uint8_t* dec_aux, int dec_rank) {
+    using Cfg = DecodeCfg<D>;
+    const int warp = threadIdx.x >> 5, lane = lane_id();
+    if (warp < kDecodeProducerWarps) {
+        if (lane < kStreamsPerProducer) {
+            const int s = warp * kStreamsPerProducer + lane;
+            const int dec_ctas = p.decode_workers / kDecodeWarps;
+            decode_producer<D>(p, tmQd, tmK, tmV, tiles + s * Cfg::kStreamBytes, dec_aux + s * Cfg::kAuxBytes,
+                               dec_rank >= 0 ? s * dec_ctas + dec_rank : -1);
+        }
+    } else {
+        const int s = warp - kDecodeProducerWarps;
+        decode_consumer<D>(p, tiles + s * Cfg::kStreamBytes, dec_aux + s * Cfg::kAuxBytes);
+    }
 }
 
 }  // namespace pa

@@ -119,17 +119,17 @@ constexpr int kTileRegion = 224 * 1024;
 constexpr int kCtrlBytes = 256;
 constexpr int kAttnSmemBytes = 1024 + kTileRegion + kCtrlBytes + kDecodeWarps * 192;
 static_assert(kAttnSmemBytes <= 232448, "attention kernel shared memory");
-static_assert(kDecodeWarps * DecodeCfg<128>::kRingBytes <= kTileRegion, "decode rings fit the tile region");
+static_assert(kDecodeWarps * DecodeCfg<128>::kStreamBytes <= kTileRegion, "decode streams fit the tile region");
+static_assert(kDecodeWarps * DecodeCfg<256>::kStreamBytes <= kTileRegion, "decode streams fit the tile region");
 
 template <int D, bool kPinTmem>
 __global__ void __launch_bounds__(kAttnThreads, 1)
-pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
-                    const __grid_constant__ CUtensorMap tmV) {
+pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmQd,
+                    const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     PrefillCtrl* ctrl = reinterpret_cast<PrefillCtrl*>(tiles + kTileRegion);
     uint8_t* dec_aux = tiles + kTileRegion + kCtrlBytes;
-    const int warp = threadIdx.x >> 5;
     const PlanView& pl = p.plan;
     if (threadIdx.x == 0) {
         tma_prefetch_desc(&tmK);
@@ -137,14 +137,17 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
         if (pl.n_units > 0) {
             tma_prefetch_desc(&tmQ);
             prefill_init_barriers(ctrl);
-            fence_mbar_init();
-            fence_proxy_async();
         }
+        if (pl.n_bundles > 0) {
+            tma_prefetch_desc(&tmQd);
+            decode_init_barriers<D>(dec_aux);
+        }
+        fence_mbar_init();
+        fence_proxy_async();
     }
     __syncthreads();
     const bool starts_prefill = (int)blockIdx.x < p.prefill_ctas;
     const int dec_rank = (int)blockIdx.x - p.prefill_ctas;       // rank among the initial decode CTAs
-    const int dec_ctas = p.decode_workers / kDecodeWarps;
 #pragma unroll 1
     for (int pass = 0; pass < 2; ++pass) {
         const bool do_prefill = (pass == 0) == starts_prefill;
@@ -153,12 +156,8 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
             if (pl.n_units > 0 && (starts_prefill || pl.n_units > p.prefill_ctas))
                 prefill_role<D, kPinTmem>(p, &tmQ, &tmK, &tmV, tiles, ctrl, starts_prefill ? (int)blockIdx.x : -1);
         } else {
-            if (pl.n_bundles > 0 && (!starts_prefill || pl.n_bundles > p.decode_workers) && warp < kDecodeWarps) {
-                // interleave so that the first dec_ctas bundles land on distinct SMs
-                const int first = starts_prefill ? -1 : warp * dec_ctas + dec_rank;
-                decode_worker<D>(p, &tmK, &tmV, tiles + warp * DecodeCfg<D>::kRingBytes, dec_aux + warp * DecodeCfg<D>::kAuxBytes,
-                                 first);
-            }
+            if (pl.n_bundles > 0 && (!starts_prefill || pl.n_bundles > p.decode_workers))
+                decode_role<D>(p, &tmQd, &tmK, &tmV, tiles, dec_aux, starts_prefill ? -1 : dec_rank);
         }
         __syncthreads();
     }
@@ -207,13 +206,14 @@ cudaError_t launch_attention(const AttnLaunch& a, cudaStream_t stream, int* laun
     const int grid_ctas = a.decode_ctas + a.prefill_ctas;
     if (grid_ctas > 0) {
         dim3 grid(grid_ctas), block(kAttnThreads);
-        const CUtensorMap& tq = a.tmQ ? *a.tmQ : *a.tmK;   // unused when there are no prefill units
+        const CUtensorMap& tq = a.tmQ ? *a.tmQ : *a.tmK;    // unused when there are no prefill units
+        const CUtensorMap& tqd = a.tmQd ? *a.tmQd : *a.tmK;  // unused when there are no decode bundles
         if (a.sh.D == 128) {
-            if (a.p_in_tmem) pa_attention_kernel<128, true><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, *a.tmK, *a.tmV);
-            else pa_attention_kernel<128, false><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, *a.tmK, *a.tmV);
+            if (a.p_in_tmem) pa_attention_kernel<128, true><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV);
+            else pa_attention_kernel<128, false><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV);
         } else {
-            if (a.p_in_tmem) pa_attention_kernel<256, true><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, *a.tmK, *a.tmV);
-            else pa_attention_kernel<256, false><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, *a.tmK, *a.tmV);
+            if (a.p_in_tmem) pa_attention_kernel<256, true><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV);
+            else pa_attention_kernel<256, false><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV);
         }
         ++launches;
         e = cudaGetLastError();

@@ -36,6 +36,7 @@ struct AttnLaunch {
     int32_t p_in_tmem;       // prefill variant: P staged in TMEM (1) or shared memory (0)
     int32_t n_simple_tiles;  // tiles routed to the plain kernel (debug)
     const CUtensorMap* tmQ;  // host copy of the query tensor map (null without prefill units)
+    const CUtensorMap* tmQd; // query tensor map of the decode role: [n_tok*Hq, D], box = G rows x 64 columns (null without decode bundles)
     const CUtensorMap* tmK;  // host copies of the pool tensor maps
     const CUtensorMap* tmV;
 };
