@@ -40,6 +40,7 @@ struct pa_ctx {
     const void* tm_qd_ptr = nullptr;
     int32_t tm_qd_ntok = -1;
     CUtensorMap tmK{}, tmV{}, tmQ{}, tmQd{};
+    TailMaps tails{};   // K and V pool maps with 8/4/2/1-row boxes
     // timer
     cudaEvent_t t0 = nullptr, t1 = nullptr;
     std::map<int, std::map<int, std::vector<double>>> samples;  // r per-mille -> n_tok -> seconds
@@ -68,7 +69,8 @@ int env_int(const char* name, int dflt) {
 }
 
 // pool[num_blocks][Hkv][16][D] bf16 -> 4-D tensor map, box = 64 columns x 16 tokens of one (block, head), 128B swizzle
-int32_t make_pool_map(pa_ctx* ctx, const void* pool, CUtensorMap* out) {
+// rows < 16: the same tensor with a shorter box, used to fetch only the filled rows of a sequence's last block
+int32_t make_pool_map(pa_ctx* ctx, const void* pool, CUtensorMap* out, int rows = kBlock) {
     if (!g_encode) {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult qres;
@@ -80,7 +82,7 @@ int32_t make_pool_map(pa_ctx* ctx, const void* pool, CUtensorMap* out) {
     const cuuint64_t D = c.head_dim, Hkv = c.num_kv_heads;
     cuuint64_t dims[4] = {D, (cuuint64_t)kBlock, Hkv, (cuuint64_t)c.num_blocks};
     cuuint64_t strides[3] = {D * 2, (cuuint64_t)kBlock * D * 2, Hkv * kBlock * D * 2};
-    cuuint32_t box[4] = {64, (cuuint32_t)kBlock, 1, 1};
+    cuuint32_t box[4] = {64, (cuuint32_t)rows, 1, 1};
     cuuint32_t estr[4] = {1, 1, 1, 1};
     CUresult r = g_encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(pool), dims, strides, box, estr,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -412,11 +414,13 @@ int32_t pa_batch_attention(pa_ctx* ctx, const void* q, const void* k_pool, const
         return fail(ctx, PA_ERR_INVALID, "pa_batch_attention: softmax_scale must be positive and finite");
     if (ctx->tm_k_ptr != k_pool) {
         int32_t rc = make_pool_map(ctx, k_pool, &ctx->tmK);
+        for (int i = 0; i < 4 && rc == PA_OK; ++i) rc = make_pool_map(ctx, k_pool, &ctx->tails.k[i], 8 >> i);
         if (rc != PA_OK) return rc;
         ctx->tm_k_ptr = k_pool;
     }
     if (ctx->tm_v_ptr != v_pool) {
         int32_t rc = make_pool_map(ctx, v_pool, &ctx->tmV);
+        for (int i = 0; i < 4 && rc == PA_OK; ++i) rc = make_pool_map(ctx, v_pool, &ctx->tails.v[i], 8 >> i);
         if (rc != PA_OK) return rc;
         ctx->tm_v_ptr = v_pool;
     }
@@ -445,6 +449,7 @@ int32_t pa_batch_attention(pa_ctx* ctx, const void* q, const void* k_pool, const
     a.tmQ = ctx->view.n_units > 0 ? &ctx->tmQ : nullptr;
     a.tmQd = ctx->view.n_bundles > 0 ? &ctx->tmQd : nullptr;
     a.tmK = &ctx->tmK; a.tmV = &ctx->tmV;
+    a.tails = &ctx->tails;
     int launches = 0;
     cudaError_t e = launch_attention(a, static_cast<cudaStream_t>(stream), &launches);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "pa_batch_attention");

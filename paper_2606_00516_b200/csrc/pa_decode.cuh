@@ -22,6 +22,7 @@
 #pragma once
 #include "pa_common.cuh"
 #include "pa_internal.h"
+#include "pa_launch.h"
 
 namespace pa {
 
@@ -73,8 +74,8 @@ __device__ __forceinline__ void decode_init_barriers(uint8_t* dec_aux) {
 // ------------------------------------------------------------------------------------------------
 template <int D>
 __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUtensorMap* tmQd, const CUtensorMap* tmK,
-                                                const CUtensorMap* tmV, uint8_t* stream_mem, uint8_t* aux,
-                                                int first_bundle) {
+                                                const CUtensorMap* tmV, const TailMaps* tails, uint8_t* stream_mem,
+                                                uint8_t* aux, int first_bundle) {
     using Cfg = DecodeCfg<D>;
     constexpr int R = Cfg::kRing, FQ = Cfg::kFifo, H = Cfg::kHalves;
     const PlanView& pl = p.plan;
@@ -88,22 +89,43 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
     int next_bundle = first_bundle;
     if (next_bundle < 0) next_bundle = p.decode_workers + atomicAdd(&pl.queue[0], 1);
     int item = 0, item_end = 0;
-    for (;;) {
-        if (item >= item_end) {
-            if (next_bundle >= pl.n_bundles) break;
+    auto next_item = [&]() -> int {    // index of the stream's next item, -1 when the bundles are exhausted
+        while (item >= item_end) {
+            if (next_bundle >= pl.n_bundles) return -1;
             item = __ldg(pl.bundle_start + next_bundle);
             item_end = __ldg(pl.bundle_start + next_bundle + 1);
             next_bundle = p.decode_workers + atomicAdd(&pl.queue[0], 1);   // result is needed one bundle later
-            continue;
+        }
+        return item++;
+    };
+    // Two-deep software pipeline over items so that no load is waited on where it is issued:
+    //   stage 2: descriptor of item i+2 in flight;  stage 1: descriptor of item i+1 arrived, its first block id in flight.
+    int4 a1 = make_int4(0, 0, 0, 0), b1 = a1, a2 = a1, b2 = a1;
+    int blkid1 = 0;
+    int i2 = next_item();
+    if (i2 >= 0) { a2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2)); b2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2) + 1); }
+    bool v1 = i2 >= 0;
+    a1 = a2; b1 = b2;
+    if (v1) {
+        blkid1 = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z);
+        i2 = next_item();
+        if (i2 >= 0) { a2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2)); b2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2) + 1); }
+    }
+    while (v1) {
+        const int4 a = a1, b = b1;
+        int blkid = blkid1;
+        // ---- advance the pipeline
+        v1 = i2 >= 0;
+        if (v1) {
+            a1 = a2; b1 = b2;
+            blkid1 = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z);
+            i2 = next_item();
+            if (i2 >= 0) { a2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2)); b2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2) + 1); }
         }
         // ---- open the item: descriptor + Q rows into the fifo entry
-        const int4* src = reinterpret_cast<const int4*>(pl.items + item);
-        const int4 a = __ldg(src), b = __ldg(src + 1);
-        ++item;
-        const int seq = a.x, kvh = a.y, blk_end = a.w;
+        const int seq = a.x, kvh = a.y, blk_end = a.w, kv_len = b.x;
         int blk = a.z;
         const int32_t* bt = p.block_tables + (int64_t)seq * p.max_blocks_per_seq;
-        int blkid = __ldg(bt + blk);
         {
             const uint32_t fs = i_iss % FQ;
             mbar_wait(bar + Cfg::kOffFEmpty + 8 * fs, ((i_iss / FQ) & 1u) ^ 1u);
@@ -121,6 +143,7 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
         // ---- stream the K and V tiles of the item's blocks
         while (blk < blk_end) {
             const int cur = blkid;
+            const int nvalid = min(kBlock, kv_len - blk * kBlock);   // filled rows of this block
             ++blk;
             if (blk < blk_end) blkid = __ldg(bt + blk);   // prefetch the next block id behind this block's issue
 #pragma unroll
@@ -130,9 +153,25 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
                     const uint32_t slot = u_iss % R;
                     mbar_wait(bar + Cfg::kOffEmpty + 8 * slot, ((u_iss / R) & 1u) ^ 1u);
                     const uint32_t full = bar + 8 * slot, dst = ring_u32 + slot * Cfg::kUnit;
-                    mbar_expect_tx(full, Cfg::kUnit);
-                    tma_load_4d_hint(dst, isV ? tmV : tmK, full, h * 128, 0, kvh, cur, pol);
-                    tma_load_4d_hint(dst + 2048, isV ? tmV : tmK, full, h * 128 + 64, 0, kvh, cur, pol);
+                    if (nvalid == kBlock) {
+                        mbar_expect_tx(full, Cfg::kUnit);
+                        tma_load_4d_hint(dst, isV ? tmV : tmK, full, h * 128, 0, kvh, cur, pol);
+                        tma_load_4d_hint(dst + 2048, isV ? tmV : tmK, full, h * 128 + 64, 0, kvh, cur, pol);
+                    } else {
+                        // partly filled last block: rows [0, nvalid) as 8 + 4 + 2 + 1 row boxes (same swizzle phase:
+                        // the 128B pattern depends on the shared-memory address, rows are 128 B apart)
+                        mbar_expect_tx(full, nvalid * 256);
+                        int r0 = 0;
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            if (nvalid & (8 >> i)) {
+                                const CUtensorMap* tm = isV ? &tails->v[i] : &tails->k[i];
+                                tma_load_4d_hint(dst + r0 * 128, tm, full, h * 128, r0, kvh, cur, pol);
+                                tma_load_4d_hint(dst + 2048 + r0 * 128, tm, full, h * 128 + 64, r0, kvh, cur, pol);
+                                r0 += 8 >> i;
+                            }
+                        }
+                    }
                     ++u_iss;
                 }
             }
@@ -302,11 +341,13 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
                 constexpr int VPL = D / 32;                  // floats per lane
                 for (int hh = 0; hh < G; ++hh) {
                     float M = -INFINITY;
+#pragma unroll 4
                     for (int i = 0; i < ci.n_parts; ++i)
                         M = fmaxf(M, __ldcg(&pl.part_ml[(ci.part_base + i) * kMaxGroup + hh]).x);
                     float L = 0.f, acc[VPL];
 #pragma unroll
                     for (int k = 0; k < VPL; ++k) acc[k] = 0.f;
+#pragma unroll 4
                     for (int i = 0; i < ci.n_parts; ++i) {
                         const float2 ml = __ldcg(&pl.part_ml[(ci.part_base + i) * kMaxGroup + hh]);
                         const float w = fast_exp2(ml.x - M);
@@ -339,14 +380,15 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
 // the first bundles land on distinct SMs); dec_rank < 0: late joiner, every bundle comes from the queue.
 template <int D>
 __device__ __forceinline__ void decode_role(const AttnParams& p, const CUtensorMap* tmQd, const CUtensorMap* tmK,
-                                            const CUtensorMap* tmV, uint8_t* tiles, uint8_t* dec_aux, int dec_rank) {
+                                            const CUtensorMap* tmV, const TailMaps* tails, uint8_t* tiles, uint8_t* dec_aux,
+                                            int dec_rank) {
     using Cfg = DecodeCfg<D>;
     const int warp = threadIdx.x >> 5, lane = lane_id();
     if (warp < kDecodeProducerWarps) {
         if (lane < kStreamsPerProducer) {
             const int s = warp * kStreamsPerProducer + lane;
             const int dec_ctas = p.decode_workers / kDecodeWarps;
-            decode_producer<D>(p, tmQd, tmK, tmV, tiles + s * Cfg::kStreamBytes, dec_aux + s * Cfg::kAuxBytes,
+            decode_producer<D>(p, tmQd, tmK, tmV, tails, tiles + s * Cfg::kStreamBytes, dec_aux + s * Cfg::kAuxBytes,
                                dec_rank >= 0 ? s * dec_ctas + dec_rank : -1);
         }
     } else {

@@ -125,7 +125,8 @@ static_assert(kDecodeWarps * DecodeCfg<256>::kStreamBytes <= kTileRegion, "decod
 template <int D, bool kPinTmem>
 __global__ void __launch_bounds__(kAttnThreads, 1)
 pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmQd,
-                    const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV) {
+                    const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                    const __grid_constant__ TailMaps tails) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     PrefillCtrl* ctrl = reinterpret_cast<PrefillCtrl*>(tiles + kTileRegion);
@@ -157,7 +158,7 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
                 prefill_role<D, kPinTmem>(p, &tmQ, &tmK, &tmV, tiles, ctrl, starts_prefill ? (int)blockIdx.x : -1);
         } else {
             if (pl.n_bundles > 0 && (!starts_prefill || pl.n_bundles > p.decode_workers))
-                decode_role<D>(p, &tmQd, &tmK, &tmV, tiles, dec_aux, starts_prefill ? -1 : dec_rank);
+                decode_role<D>(p, &tmQd, &tmK, &tmV, &tails, tiles, dec_aux, starts_prefill ? -1 : dec_rank);
         }
         __syncthreads();
     }
@@ -209,11 +210,11 @@ cudaError_t launch_attention(const AttnLaunch& a, cudaStream_t stream, int* laun
         const CUtensorMap& tq = a.tmQ ? *a.tmQ : *a.tmK;    // unused when there are no prefill units
         const CUtensorMap& tqd = a.tmQd ? *a.tmQd : *a.tmK;  // unused when there are no decode bundles
         if (a.sh.D == 128) {
-            if (a.p_in_tmem) pa_attention_kernel<128, true><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV);
-            else pa_attention_kernel<128, false><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV);
+            if (a.p_in_tmem) pa_attention_kernel<128, true><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV, *a.tails);
+            else pa_attention_kernel<128, false><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV, *a.tails);
         } else {
-            if (a.p_in_tmem) pa_attention_kernel<256, true><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV);
-            else pa_attention_kernel<256, false><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV);
+            if (a.p_in_tmem) pa_attention_kernel<256, true><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV, *a.tails);
+            else pa_attention_kernel<256, false><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV, *a.tails);
         }
         ++launches;
         e = cudaGetLastError();

@@ -20,6 +20,12 @@ cudaError_t launch_kv_append(const LaunchShape& sh, const void* k_new, const voi
 cudaError_t launch_kv_gather(const LaunchShape& sh, const void* k_pool, const void* v_pool, const int32_t* table_row,
                              int32_t kv_len, void* k_out, void* v_out, cudaStream_t stream);
 
+// Pool tensor maps whose boxes hold 8, 4, 2, 1 token rows (index 0..3): the filled rows of a partly filled last
+// block are fetched as the binary decomposition of their count, so decode never reads slots that hold no token.
+struct TailMaps {
+    CUtensorMap k[4], v[4];
+};
+
 struct AttnLaunch {
     LaunchShape sh;
     const void* q;
@@ -39,6 +45,7 @@ struct AttnLaunch {
     const CUtensorMap* tmQd; // query tensor map of the decode role: [n_tok*Hq, D], box = G rows x 64 columns (null without decode bundles)
     const CUtensorMap* tmK;  // host copies of the pool tensor maps
     const CUtensorMap* tmV;
+    const TailMaps* tails;
 };
 
 // Set opt-in shared memory sizes once per process/device.
