@@ -40,7 +40,7 @@ struct pa_ctx {
     const void* tm_qd_ptr = nullptr;
     int32_t tm_qd_ntok = -1;
     CUtensorMap tmK{}, tmV{}, tmQ{}, tmQd{};
-    TailMaps tails{};   // K and V pool maps with 8/4/2/1-row boxes
+    TailMaps tails{};   // decode views of the K and V pools (16/8/4/2/1-row boxes)
     // timer
     cudaEvent_t t0 = nullptr, t1 = nullptr;
     std::map<int, std::map<int, std::vector<double>>> samples;  // r per-mille -> n_tok -> seconds
@@ -88,6 +88,21 @@ int32_t make_pool_map(pa_ctx* ctx, const void* pool, CUtensorMap* out, int rows 
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(ctx, PA_ERR_CUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
+    return PA_OK;
+}
+
+// decode view of the pool (pa_launch.h TailMaps): 5-D, box = 64 columns x `rows` tokens x `planes` column planes
+int32_t make_pool_map5(pa_ctx* ctx, const void* pool, CUtensorMap* out, int rows, int planes) {
+    const pa_config& c = ctx->cfg;
+    const cuuint64_t D = c.head_dim, Hkv = c.num_kv_heads;
+    cuuint64_t dims[5] = {64, (cuuint64_t)kBlock, D / 64, Hkv, (cuuint64_t)c.num_blocks};
+    cuuint64_t strides[4] = {D * 2, 128, (cuuint64_t)kBlock * D * 2, Hkv * kBlock * D * 2};
+    cuuint32_t box[5] = {64, (cuuint32_t)rows, (cuuint32_t)planes, 1, 1};
+    cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    CUresult r = g_encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void*>(pool), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(ctx, PA_ERR_CUDA, "cuTensorMapEncodeTiled(pool, 5-D) failed (" + std::to_string((int)r) + ")");
     return PA_OK;
 }
 
@@ -160,7 +175,7 @@ int32_t pa_create(pa_ctx** out, const pa_config* cfg) {
     }
     // ---- workspace layout
     ctx->max_workers = ctx->num_sms * kDecodeWarps;
-    ctx->max_bundles = ctx->max_workers * 4 + 8;
+    ctx->max_bundles = ctx->max_workers * 5 + 8;   // k <= 4 bundles per worker; unsplit short groups close bundles up to 1/8 early
     ctx->max_items = cfg->max_seqs * cfg->num_kv_heads + ctx->max_bundles + 8;
     ctx->max_split = 2 * ctx->max_bundles;
     ctx->max_tiles = cfg->max_tokens / kQTile + cfg->max_seqs + 1;
@@ -300,6 +315,23 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
             const int32_t nblk = (kv_len + kBlock - 1) / kBlock;
             for (int g = 0; g < Hkv; ++g) {
                 int32_t pos = 0, first_item = n_items;
+                if ((nblk <= 2 || (int64_t)nblk * 4 <= target) && cur + nblk > target) {
+                    // a short group is never cut (partials + merge would cost more than the imbalance, which is
+                    // bounded by a quarter bundle): it goes whole into this bundle or the next, whichever ends
+                    // nearer the target
+                    if (cur + nblk - target > target - cur) {
+                        bundle_start.push_back(n_items);
+                        cur = 0;
+                    }
+                    if (n_items >= ctx->max_items) return fail(ctx, PA_ERR_INVALID, "pa_plan: decode item list overflow");
+                    items[n_items++] = DecItem{s, g, 0, nblk, kv_len, -1, 0, 1};
+                    cur += nblk;
+                    if (cur >= target) {
+                        bundle_start.push_back(n_items);
+                        cur = 0;
+                    }
+                    continue;
+                }
                 while (pos < nblk) {
                     const int32_t take = (int32_t)std::min<int64_t>(nblk - pos, target - cur);
                     if (n_items >= ctx->max_items) return fail(ctx, PA_ERR_INVALID, "pa_plan: decode item list overflow");
@@ -414,13 +446,13 @@ int32_t pa_batch_attention(pa_ctx* ctx, const void* q, const void* k_pool, const
         return fail(ctx, PA_ERR_INVALID, "pa_batch_attention: softmax_scale must be positive and finite");
     if (ctx->tm_k_ptr != k_pool) {
         int32_t rc = make_pool_map(ctx, k_pool, &ctx->tmK);
-        for (int i = 0; i < 4 && rc == PA_OK; ++i) rc = make_pool_map(ctx, k_pool, &ctx->tails.k[i], 8 >> i);
+        for (int i = 0; i < 5 && rc == PA_OK; ++i) rc = make_pool_map5(ctx, k_pool, &ctx->tails.k[i], 16 >> i, i == 0 ? 2 : 1);
         if (rc != PA_OK) return rc;
         ctx->tm_k_ptr = k_pool;
     }
     if (ctx->tm_v_ptr != v_pool) {
         int32_t rc = make_pool_map(ctx, v_pool, &ctx->tmV);
-        for (int i = 0; i < 4 && rc == PA_OK; ++i) rc = make_pool_map(ctx, v_pool, &ctx->tails.v[i], 8 >> i);
+        for (int i = 0; i < 5 && rc == PA_OK; ++i) rc = make_pool_map5(ctx, v_pool, &ctx->tails.v[i], 16 >> i, i == 0 ? 2 : 1);
         if (rc != PA_OK) return rc;
         ctx->tm_v_ptr = v_pool;
     }

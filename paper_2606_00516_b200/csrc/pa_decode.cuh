@@ -101,24 +101,26 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
     // Two-deep software pipeline over items so that no load is waited on where it is issued:
     //   stage 2: descriptor of item i+2 in flight;  stage 1: descriptor of item i+1 arrived, its first block id in flight.
     int4 a1 = make_int4(0, 0, 0, 0), b1 = a1, a2 = a1, b2 = a1;
-    int blkid1 = 0;
+    int blkid1 = 0, blkid1n = 0;      // ids of the first two blocks of the stage-1 item
     int i2 = next_item();
     if (i2 >= 0) { a2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2)); b2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2) + 1); }
     bool v1 = i2 >= 0;
     a1 = a2; b1 = b2;
     if (v1) {
         blkid1 = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z);
+        if (a1.z + 1 < a1.w) blkid1n = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z + 1);
         i2 = next_item();
         if (i2 >= 0) { a2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2)); b2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2) + 1); }
     }
     while (v1) {
         const int4 a = a1, b = b1;
-        int blkid = blkid1;
+        int blkid = blkid1, blkid_n = blkid1n;
         // ---- advance the pipeline
         v1 = i2 >= 0;
         if (v1) {
             a1 = a2; b1 = b2;
             blkid1 = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z);
+            if (a1.z + 1 < a1.w) blkid1n = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z + 1);
             i2 = next_item();
             if (i2 >= 0) { a2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2)); b2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2) + 1); }
         }
@@ -145,7 +147,8 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
             const int cur = blkid;
             const int nvalid = min(kBlock, kv_len - blk * kBlock);   // filled rows of this block
             ++blk;
-            if (blk < blk_end) blkid = __ldg(bt + blk);   // prefetch the next block id behind this block's issue
+            blkid = blkid_n;
+            if (blk + 1 < blk_end) blkid_n = __ldg(bt + blk + 1);   // block ids are fetched two blocks ahead of their use
 #pragma unroll
             for (int isV = 0; isV < 2; ++isV) {
 #pragma unroll
@@ -155,20 +158,20 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
                     const uint32_t full = bar + 8 * slot, dst = ring_u32 + slot * Cfg::kUnit;
                     if (nvalid == kBlock) {
                         mbar_expect_tx(full, Cfg::kUnit);
-                        tma_load_4d_hint(dst, isV ? tmV : tmK, full, h * 128, 0, kvh, cur, pol);
-                        tma_load_4d_hint(dst + 2048, isV ? tmV : tmK, full, h * 128 + 64, 0, kvh, cur, pol);
+                        tma_load_5d_hint(dst, isV ? &tails->v[0] : &tails->k[0], full, 0, 0, 2 * h, kvh, cur, pol);
                     } else {
-                        // partly filled last block: rows [0, nvalid) as 8 + 4 + 2 + 1 row boxes (same swizzle phase:
-                        // the 128B pattern depends on the shared-memory address, rows are 128 B apart)
+                        // partly filled last block: rows [0, nvalid) as 8 + 4 + 2 + 1 row boxes of ONE column plane each
+                        // (a short two-plane box would put plane 1 at rows·128 B, not at the slot's 2048 B plane offset;
+                        // the 128B swizzle pattern depends on the shared-memory address only, rows are 128 B apart)
                         mbar_expect_tx(full, nvalid * 256);
                         int r0 = 0;
 #pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            if (nvalid & (8 >> i)) {
+                        for (int i = 1; i < 5; ++i) {
+                            if (nvalid & (16 >> i)) {
                                 const CUtensorMap* tm = isV ? &tails->v[i] : &tails->k[i];
-                                tma_load_4d_hint(dst + r0 * 128, tm, full, h * 128, r0, kvh, cur, pol);
-                                tma_load_4d_hint(dst + 2048 + r0 * 128, tm, full, h * 128 + 64, r0, kvh, cur, pol);
-                                r0 += 8 >> i;
+                                tma_load_5d_hint(dst + r0 * 128, tm, full, 0, r0, 2 * h, kvh, cur, pol);
+                                tma_load_5d_hint(dst + 2048 + r0 * 128, tm, full, 0, r0, 2 * h + 1, kvh, cur, pol);
+                                r0 += 16 >> i;
                             }
                         }
                     }
@@ -184,6 +187,73 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
         const uint32_t d = smem_u32(aux + Cfg::kOffDesc + 32 * fs);
         asm volatile("st.shared.b32 [%0], %1;" ::"r"(d), "r"(-1) : "memory");
         mbar_arrive(bar + Cfg::kOffFFull + 8 * fs);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a6 merge of one split (sequence, KV head) group by one warp: m = max m_i, l = Σ l_i 2^{m_i-m},
+// o = Σ o_i 2^{m_i-m} / l.  Lane (i, h) = (lane / 8, lane % 8) owns the (m, l) of part c0 + i, head h, so the
+// statistics of four parts arrive with ONE coalesced load and reduce with two shuffles; the partial outputs
+// of those four parts are then fetched for all heads at once (loads of heads >= G are clamped duplicates, so
+// that no load waits on a branch) — the merge costs a few L2 round trips, not a few per head.
+// ------------------------------------------------------------------------------------------------
+template <int D, int GG>
+__device__ __forceinline__ void decode_merge(const AttnParams& p, const DecItem& ci, int q_row, int h0, int lane) {
+    constexpr int VPL = D / 32;                  // floats per lane
+    const PlanView& pl = p.plan;
+    const int G = p.G, np = ci.n_parts;
+    const int pi = lane >> 3, hl = lane & 7;
+    const float2* ml_base = pl.part_ml + (int64_t)ci.part_base * kMaxGroup;
+    float M = -INFINITY;
+    for (int c0 = 0; c0 < np; c0 += 4)
+        if (c0 + pi < np) M = fmaxf(M, __ldcg(ml_base + (c0 + pi) * kMaxGroup + hl).x);
+    M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, 8));
+    M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, 16));          // max of head hl over all parts, on every lane
+    float L = 0.f, acc[GG][VPL];
+#pragma unroll
+    for (int h = 0; h < GG; ++h)
+#pragma unroll
+        for (int k = 0; k < VPL; ++k) acc[h][k] = 0.f;
+    for (int c0 = 0; c0 < np; c0 += 4) {
+        float w = 0.f;
+        if (c0 + pi < np) {
+            const float2 ml = __ldcg(ml_base + (c0 + pi) * kMaxGroup + hl);
+            w = fast_exp2(ml.x - M);
+            L += ml.y * w;
+        }
+        const int nk = min(4, np - c0);
+        for (int k = 0; k < nk; ++k) {
+            const float* src = pl.part_o + (int64_t)(ci.part_base + c0 + k) * G * D + lane * VPL;
+            float4 v[GG][VPL / 4];
+#pragma unroll
+            for (int h = 0; h < GG; ++h)
+#pragma unroll
+                for (int x = 0; x < VPL / 4; ++x)
+                    v[h][x] = __ldcg(reinterpret_cast<const float4*>(src + min(h, G - 1) * D) + x);
+#pragma unroll
+            for (int h = 0; h < GG; ++h) {
+                const float wk = __shfl_sync(0xffffffffu, w, k * 8 + h);
+#pragma unroll
+                for (int x = 0; x < VPL / 4; ++x) {
+                    acc[h][4 * x] += wk * v[h][x].x; acc[h][4 * x + 1] += wk * v[h][x].y;
+                    acc[h][4 * x + 2] += wk * v[h][x].z; acc[h][4 * x + 3] += wk * v[h][x].w;
+                }
+            }
+        }
+    }
+    L += __shfl_xor_sync(0xffffffffu, L, 8);
+    L += __shfl_xor_sync(0xffffffffu, L, 16);
+#pragma unroll
+    for (int h = 0; h < GG; ++h) {
+        const float inv = 1.f / __shfl_sync(0xffffffffu, L, h);
+        if (h < G) {
+            uint32_t packed[VPL / 2];
+#pragma unroll
+            for (int k = 0; k < VPL / 2; ++k) packed[k] = pack_bf16x2(acc[h][2 * k] * inv, acc[h][2 * k + 1] * inv);
+            uint32_t* dst = reinterpret_cast<uint32_t*>(p.out + ((int64_t)q_row * p.Hq + h0 + h) * D + lane * VPL);
+            if constexpr (VPL == 4) *reinterpret_cast<uint2*>(dst) = make_uint2(packed[0], packed[1]);
+            else *reinterpret_cast<uint4*>(dst) = make_uint4(packed[0], packed[1], packed[2], packed[3]);
+        }
     }
 }
 
@@ -338,37 +408,8 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
             if (last) {
                 // ---------------- a6 merge by the last-arriving consumer
                 __threadfence();
-                constexpr int VPL = D / 32;                  // floats per lane
-                for (int hh = 0; hh < G; ++hh) {
-                    float M = -INFINITY;
-#pragma unroll 4
-                    for (int i = 0; i < ci.n_parts; ++i)
-                        M = fmaxf(M, __ldcg(&pl.part_ml[(ci.part_base + i) * kMaxGroup + hh]).x);
-                    float L = 0.f, acc[VPL];
-#pragma unroll
-                    for (int k = 0; k < VPL; ++k) acc[k] = 0.f;
-#pragma unroll 4
-                    for (int i = 0; i < ci.n_parts; ++i) {
-                        const float2 ml = __ldcg(&pl.part_ml[(ci.part_base + i) * kMaxGroup + hh]);
-                        const float w = fast_exp2(ml.x - M);
-                        L += ml.y * w;
-                        const float4* src = reinterpret_cast<const float4*>(
-                            pl.part_o + ((int64_t)(ci.part_base + i) * G + hh) * D + lane * VPL);
-#pragma unroll
-                        for (int k = 0; k < VPL / 4; ++k) {
-                            const float4 v = __ldcg(src + k);
-                            acc[4 * k] += w * v.x; acc[4 * k + 1] += w * v.y;
-                            acc[4 * k + 2] += w * v.z; acc[4 * k + 3] += w * v.w;
-                        }
-                    }
-                    const float inv = 1.f / L;
-                    uint32_t packed[VPL / 2];
-#pragma unroll
-                    for (int k = 0; k < VPL / 2; ++k) packed[k] = pack_bf16x2(acc[2 * k] * inv, acc[2 * k + 1] * inv);
-                    uint32_t* dst = reinterpret_cast<uint32_t*>(p.out + ((int64_t)q_row * p.Hq + h0 + hh) * D + lane * VPL);
-                    if constexpr (VPL == 4) *reinterpret_cast<uint2*>(dst) = make_uint2(packed[0], packed[1]);
-                    else *reinterpret_cast<uint4*>(dst) = make_uint4(packed[0], packed[1], packed[2], packed[3]);
-                }
+                if (G <= 4) decode_merge<D, 4>(p, ci, q_row, h0, lane);
+                else decode_merge<D, 8>(p, ci, q_row, h0, lane);
                 if (lane == 0) *ctr = 0;                      // self-reset for the next launch
             }
         }

@@ -20,10 +20,14 @@ cudaError_t launch_kv_append(const LaunchShape& sh, const void* k_new, const voi
 cudaError_t launch_kv_gather(const LaunchShape& sh, const void* k_pool, const void* v_pool, const int32_t* table_row,
                              int32_t kv_len, void* k_out, void* v_out, cudaStream_t stream);
 
-// Pool tensor maps whose boxes hold 8, 4, 2, 1 token rows (index 0..3): the filled rows of a partly filled last
-// block are fetched as the binary decomposition of their count, so decode never reads slots that hold no token.
+// Pool tensor maps of the decode role: the pool viewed as the 5-D tensor [block][kv head][D/64][16 rows][64 cols]
+// (row stride 2·D bytes, 64-column plane stride 128 bytes), box = 64 columns x rows x 2 planes, so ONE tensor load
+// brings the 128-column K (or V) unit of a block-head into the ring slot as [plane][row][128 B] (128B swizzle).
+// Index 0: 16-row, two-plane box (a full block); 1..4: 8, 4, 2, 1 rows of ONE plane — the filled rows of a partly
+// filled last block are fetched as the binary decomposition of their count (per plane), so decode never reads slots
+// that hold no token.
 struct TailMaps {
-    CUtensorMap k[4], v[4];
+    CUtensorMap k[5], v[5];
 };
 
 struct AttnLaunch {
