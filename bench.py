@@ -37,6 +37,10 @@ UNIT = "tokens/s"
 R_GRID = [i / 10 for i in range(11)]
 FIT_NTOK = [512, 1024, 2048, 4096]          # DESIGN R18
 L2_FLUSH_BYTES = 512 << 20
+# dram__bytes_read.sum + dram__bytes_write.sum per pa_attention_kernel launch, mean over the 11 r-batches of C2,
+# from the ncu --set full capture summarised in profiles/ (None until that capture exists)
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+NCU_TRAFFIC_SOURCE = None
 
 
 def _peaks():
@@ -235,11 +239,17 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        # events around the attention launch of every timed step (same stream): the dominant kernel's duration,
+        # measured live inside the timed region, feeds `roofline`
+        kev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
         e0.record()
         launches = 0
         for i in range(K):
             p = preps[i % len(preps)]
-            p.step()
+            p.append()
+            kev[i][0].record()
+            p.attention()
+            kev[i][1].record()
             launches += p.launches
         e1.record()
         torch.cuda.synchronize()
@@ -247,6 +257,9 @@ def run_ours(args):
             dist.barrier()
         sec = e0.elapsed_time(e1) * 1e-3
         tokens = sum(preps[i % len(preps)].batch.n_tok for i in range(K))
+        attn_sec = [a.elapsed_time(b) * 1e-3 for a, b in kev]
+        attn_bytes = [preps[i % len(preps)].batch.algorithmic_bytes() for i in range(K)]
+        attn_roof = [_roof_seconds(preps[i % len(preps)].batch, peaks)[0] for i in range(K)]
         if world > 1:
             t = torch.tensor([sec], device=dev, dtype=torch.float64)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -265,12 +278,21 @@ def run_ours(args):
             # ---------------- per-r table at the config's n_tok (cold L2 via flush), roofline fractions
             for p in preps:
                 sweep.append(_point(p, peaks, args.reps, W, flush))
-            # dominant kernel: the decode kernel timed alone on the pure-decode step (single launch per call)
+            # dominant kernel: pa_attention_kernel, the ONE launch of every batch_attention call (decode streams +
+            # tcgen05 prefill units + merge).  achieved = algorithmic bytes per launch / average launch duration,
+            # both averaged over the K timed steps; `traffic` = ncu dram bytes per launch, same average.
+            mean_bytes, mean_sec = float(np.mean(attn_bytes)), float(np.mean(attn_sec))
             dec = sweep[-1]
-            roofline = {"kernel": "pa_decode_kernel<128> (C2 r=1.0: the only kernel of that batch_attention call)",
-                        "bound": "hbm", "achieved": dec["achieved_GBps"], "peak": peaks["hbm"], "unit": "GB/s",
-                        "frac": dec["achieved_GBps"] / peaks["hbm"], "traffic": None, "peak_source": peaks["src"],
-                        "launch_us": dec["T_attn_us_median"]}
+            roofline = {"kernel": "pa::pa_attention_kernel<128, true> (single mixed launch per step; averaged over the "
+                                  "K timed steps of the r cycle)",
+                        "bound": "hbm", "achieved": mean_bytes / mean_sec / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
+                        "frac": mean_bytes / mean_sec / 1e9 / peaks["hbm"], "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+                        "traffic_source": NCU_TRAFFIC_SOURCE, "peak_source": peaks["src"] + " (burst copy figure)",
+                        "alg_bytes_per_launch": mean_bytes, "launch_us": mean_sec * 1e6,
+                        "kernel_share_of_step": sum(attn_sec) / sec,
+                        "roofline_time_frac": float(np.sum(attn_roof) / np.sum(attn_sec)),
+                        "pure_decode_r1": {"achieved": dec["achieved_GBps"], "frac": dec["achieved_GBps"] / peaks["hbm"],
+                                           "launch_us": dec["T_attn_us_median"], "note": "C2 r=1.0 alone, cold L2"}}
             # ---------------- alpha/beta per r through the library's step timer (a8)
             if not args.no_fit:
                 fits = _fit_sweep(dev, W, args.reps, flush)

@@ -291,19 +291,64 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     const bool simple_all = (c.flags & PA_FLAG_DEBUG_SIMPLE) != 0;
     const int Hkv = c.num_kv_heads, D = c.head_dim, G = ctx->G;
 
+    // ---- prefill tiles (built first: the decode bundling below depends on how many CTAs prefill takes)
+    std::vector<PreTile> tile_vec;
+    for (int s = simple_all ? 0 : num_decode_seqs; s < n_seq; ++s) {
+        const int32_t ql = h_cu[s + 1] - h_cu[s];
+        for (int32_t q0 = 0; q0 < ql; q0 += kQTile) {
+            if ((int32_t)tile_vec.size() >= ctx->max_tiles) return fail(ctx, PA_ERR_INVALID, "pa_plan: tile list overflow");
+            const int32_t rows = std::min(kQTile, ql - q0);
+            tile_vec.push_back(PreTile{s, q0, rows, h_ctx[s], h_ctx[s] + ql, h_cu[s], {0, 0}});
+        }
+    }
+    const int32_t n_tiles = (int32_t)tile_vec.size();
+    // longest first: the queue then hands out units in LPT order (causal tiles late in a chunk see more keys)
+    std::stable_sort(tile_vec.begin(), tile_vec.end(), [](const PreTile& a, const PreTile& b) {
+        return a.ctx + a.q_begin + a.q_rows > b.ctx + b.q_begin + b.q_rows;
+    });
+    const int prefill_mode = simple_all ? 2 : env_int("PA_PREFILL_MODE", 0);   // 0 P in TMEM, 1 P in smem, 2 plain kernel
+    const int NQ = D == 128 ? 2 : 1;
+    const int32_t head_groups = (G + NQ - 1) / NQ;
+    const int32_t n_units = prefill_mode == 2 ? 0 : n_tiles * Hkv * head_groups;
+    const int n_dec = simple_all ? 0 : num_decode_seqs;
+    int64_t total_blocks = 0;
+    for (int s = 0; s < n_dec; ++s) total_blocks += ((int64_t)h_ctx[s] + 1 + kBlock - 1) / kBlock * Hkv;
+    // ---- CTA partition of the single launch (a7): share the SMs in proportion to the estimated CTA-time of the
+    // two roles.  Prefill: per unit a fill of ~1.5 us plus ~1.4 us per (q-head tile, KV tile) pair (measured
+    // softmax/MMA pipeline rate).  Decode: the larger of its HBM time on all SMs and the per-stream latency time
+    // (~3 us per item + bytes at ~16 GB/s per stream, 8 streams per CTA).  CTAs switch role when their own queue
+    // runs dry, so the split only has to be roughly right (measured flat within +-30 % of this choice).
+    const int sms = ctx->num_sms;
+    int32_t pre_ctas = 0;
+    if (n_units > 0 && total_blocks > 0) {
+        const int KT = D == 128 ? 128 : 64;
+        double t_pre = 0.0;   // CTA-microseconds
+        for (const PreTile& t : tile_vec) {
+            const double n_kv = std::ceil((double)(t.ctx + t.q_begin + t.q_rows) / KT);
+            t_pre += (double)Hkv * (head_groups * 1.5 + n_kv * G * 1.4);
+        }
+        const double dec_bytes = (double)total_blocks * kBlock * D * 2 * 2;
+        const double n_groups = (double)n_dec * Hkv;
+        const double t_dec = std::max(sms * dec_bytes / 6.5e12 * 1e6, n_groups * 3.0 / kDecodeWarps + dec_bytes / 16e9 / kDecodeWarps * 1e6);
+        pre_ctas = (int32_t)std::lround(sms * t_pre / (t_pre + t_dec));
+        pre_ctas = env_int("PA_PREFILL_CTAS", pre_ctas);
+        pre_ctas = std::max(1, std::min({pre_ctas, sms - 1, n_units}));
+    } else if (n_units > 0) {
+        pre_ctas = std::min(sms, n_units);
+    }
     // ---- decode bundles
     DecItem* items = reinterpret_cast<DecItem*>(ctx->h_stage);
     int32_t n_items = 0, n_bundles = 0, n_split = 0;
     std::vector<int32_t> bundle_start;
-    const int n_dec = simple_all ? 0 : num_decode_seqs;
-    int64_t total_blocks = 0;
-    for (int s = 0; s < n_dec; ++s) total_blocks += ((int64_t)h_ctx[s] + 1 + kBlock - 1) / kBlock * Hkv;
     if (total_blocks > 0) {
-        const int64_t W = ctx->max_workers;
+        // workers that start in the decode role; in a mixed launch the prefill CTAs join through the queue when
+        // their units run out, so bundles are made finer (>= 4 per worker) and the tail balances dynamically
+        const int64_t W = (int64_t)(sms - pre_ctas) * kDecodeWarps;
+        const bool mixed = pre_ctas > 0;
         const double kv_bytes = (double)total_blocks * kBlock * D * 2 * 2;
         const double part_bytes = (double)G * D * 4 * 2;
         int k = (int)std::floor(0.01 * kv_bytes / ((double)W * part_bytes));
-        k = std::max(1, std::min(4, k));
+        k = std::max(mixed ? 4 : 1, std::min(4, k));
         k = std::max(1, std::min(4, env_int("PA_BUNDLE_K", k)));
         const int64_t min_blocks = std::max(1, env_int("PA_MIN_BUNDLE_BLOCKS", 2));
         const int64_t target = std::max(min_blocks, (total_blocks + W * k - 1) / (W * k));
@@ -359,31 +404,12 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
         n_bundles = (int32_t)bundle_start.size() - 1;
         if (n_bundles > ctx->max_bundles) return fail(ctx, PA_ERR_INVALID, "pa_plan: bundle list overflow");
     }
-    // ---- prefill tiles
+    // ---- staging layout: items | bundle_start | tiles
     int64_t off_b = align_up((int64_t)n_items * sizeof(DecItem), 256);
     int32_t* h_bundles = reinterpret_cast<int32_t*>(ctx->h_stage + off_b);
     for (int32_t i = 0; i <= n_bundles && n_bundles > 0; ++i) h_bundles[i] = bundle_start[i];
     int64_t off_t = off_b + align_up((int64_t)(n_bundles + 1) * 4, 256);
-    PreTile* tiles = reinterpret_cast<PreTile*>(ctx->h_stage + off_t);
-    int32_t n_tiles = 0;
-    double pre_flops = 0.0;
-    for (int s = simple_all ? 0 : num_decode_seqs; s < n_seq; ++s) {
-        const int32_t ql = h_cu[s + 1] - h_cu[s];
-        for (int32_t q0 = 0; q0 < ql; q0 += kQTile) {
-            if (n_tiles >= ctx->max_tiles) return fail(ctx, PA_ERR_INVALID, "pa_plan: tile list overflow");
-            const int32_t rows = std::min(kQTile, ql - q0);
-            tiles[n_tiles++] = PreTile{s, q0, rows, h_ctx[s], h_ctx[s] + ql, h_cu[s], {0, 0}};
-            pre_flops += 4.0 * D * c.num_q_heads * rows * ((double)h_ctx[s] + q0 + 0.5 * rows);
-        }
-    }
-    // longest first: the queue then hands out units in LPT order (causal tiles late in a chunk see more keys)
-    std::stable_sort(tiles, tiles + n_tiles, [](const PreTile& a, const PreTile& b) {
-        return a.ctx + a.q_begin + a.q_rows > b.ctx + b.q_begin + b.q_rows;
-    });
-    const int prefill_mode = simple_all ? 2 : env_int("PA_PREFILL_MODE", 0);   // 0 P in TMEM, 1 P in smem, 2 plain kernel
-    const int NQ = D == 128 ? 2 : 1;
-    const int32_t head_groups = (G + NQ - 1) / NQ;
-    const int32_t n_units = prefill_mode == 2 ? 0 : n_tiles * Hkv * head_groups;
+    if (n_tiles > 0) std::memcpy(ctx->h_stage + off_t, tile_vec.data(), (size_t)n_tiles * sizeof(PreTile));
     const int64_t used = off_t + align_up((int64_t)n_tiles * sizeof(PreTile), 256);
 
     // ---- upload
@@ -409,22 +435,8 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     v.n_split = n_split;
     v.n_units = n_units;
     v.head_groups = head_groups;
-    // ---- CTA partition of the single launch (a7): share the SMs in proportion to the estimated
-    // tensor time of the prefill units and HBM time of the decode bundles; CTAs switch role when
-    // their own queue runs dry, so the split only has to be roughly right.
-    const int sms = ctx->num_sms;
-    int32_t pre_ctas = 0, dec_ctas = 0;
-    if (n_units > 0 && n_bundles > 0) {
-        const double t_pre = pre_flops / (0.45 * 1.4e15), t_dec = (double)total_blocks * kBlock * D * 2 * 2 / 6.5e12;
-        pre_ctas = (int32_t)std::lround(sms * t_pre / (t_pre + t_dec));
-        pre_ctas = env_int("PA_PREFILL_CTAS", pre_ctas);
-        pre_ctas = std::max(1, std::min({pre_ctas, sms - 1, n_units}));
-        dec_ctas = std::min(sms - pre_ctas, n_bundles);
-    } else if (n_units > 0) {
-        pre_ctas = std::min(sms, n_units);
-    } else if (n_bundles > 0) {
-        dec_ctas = std::min(sms, n_bundles);
-    }
+    int32_t dec_ctas = 0;
+    if (n_bundles > 0) dec_ctas = std::min(sms - pre_ctas, n_bundles);
     ctx->decode_ctas = dec_ctas;
     ctx->prefill_ctas = pre_ctas;
     ctx->p_in_tmem = prefill_mode == 0;
