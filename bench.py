@@ -39,8 +39,8 @@ FIT_NTOK = [512, 1024, 2048, 4096]          # DESIGN R18
 L2_FLUSH_BYTES = 512 << 20
 # dram__bytes_read.sum + dram__bytes_write.sum per pa_attention_kernel launch, mean over the 11 r-batches of C2,
 # from the ncu --set full capture summarised in profiles/ (None until that capture exists)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
-NCU_TRAFFIC_SOURCE = None
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 95395840.0
+NCU_TRAFFIC_SOURCE = "profiles/r1e_c2_cycle.md (ncu --set full, 11 launches of one r-cycle)"
 
 
 def _peaks():
@@ -101,6 +101,24 @@ class ClockSampler:
         ignore = {"GpuIdle", "ApplicationsClocksSetting"}
         return {"sm_mhz": float(np.median(busy)) if busy else None, "sm_max_mhz": self.max_mhz,
                 "reasons": sorted(self.reasons - ignore), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------ ranks
+def max_over_ranks(seconds: float, device=None) -> float:
+    """Replicas only: the job's time is the slowest rank's device time.  all_reduce(MAX) on the
+    process group's device (cuda for nccl, cpu for the gloo tests); identity without a process group."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(seconds)
+    t = torch.tensor([seconds], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(tokens_per_rank: int, seconds: float, world: int) -> float:
+    """Whole-job tokens/s of `world` identical replicas (weak scaling): Σ tokens ÷ max-over-ranks time."""
+    return world * tokens_per_rank / seconds
 
 
 # ------------------------------------------------------------------------------------------------ ours
@@ -184,32 +202,39 @@ def _point(prep, peaks, reps, warmup, flush):
             "split_items": prep.pa.plan_info(2), "prefill_tiles": prep.pa.plan_info(3)}
 
 
-def _cpu_baseline(dev, seconds_budget=20.0):
-    """The oracle, as it stands, on this host's cores: one C2 r=0.5 step (bounded sample)."""
+def _cpu_baseline(dev, seconds_budget=10.0):
+    """The oracle, as it stands, on this host's cores: whole C2 steps (kv_append + attention of all 2048 rows),
+    cycling r = 0.0, 0.1, ... like the timed region, until `seconds_budget` seconds of CPU work are done."""
     import torch
     import oracle
     from paper_2606_00516_b200.synth import device as sdev
     from paper_2606_00516_b200.synth import workloads
-    batch = workloads.config2(0.5)
-    db = sdev.materialise(batch, dev)
-    torch.cuda.synchronize()
-    sh = batch.shape
-    osh = oracle.PagedShape(sh.num_q_heads, sh.num_kv_heads, sh.head_dim, sh.block_size)
-    q, kn, vn = sdev.bits(db.q), sdev.bits(db.k_new), sdev.bits(db.v_new)
-    kp, vp = sdev.bits(db.k_pool), sdev.bits(db.v_pool)
-    del db
     cores = os.cpu_count() or 1
-    # bounded sample: ONE full step of the r = 0.5 batch (all 2048 token rows; ≈ 10–30 s of CPU work)
-    nd = batch.n_decode_tok
-    rows = np.arange(batch.n_tok, dtype=np.int64)
-    t0 = time.perf_counter()
-    oracle.kv_append(osh, kn, vn, kp, vp, batch.cu_seqlens_q, batch.context_lens, batch.block_tables)
-    oracle.attention(osh, q, kp, vp, batch.cu_seqlens_q, batch.context_lens, batch.block_tables, batch.softmax_scale,
-                     rows=rows, n_threads=cores)
-    dt = time.perf_counter() - t0
-    return {"value": len(rows) / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
-            "sample": f"C2 r=0.5 batch (seed 205): kv_append of all 2048 tokens + attention of {len(rows)} rows "
-                      f"({nd} decode rows at ctx 16 + {batch.n_tok - nd} prefill rows of 512-token prompts), fp64 oracle, {cores} threads"}
+    hosts = []
+    for r in R_GRID:
+        batch = workloads.config2(r)
+        db = sdev.materialise(batch, dev)
+        torch.cuda.synchronize()
+        sh = batch.shape
+        osh = oracle.PagedShape(sh.num_q_heads, sh.num_kv_heads, sh.head_dim, sh.block_size)
+        hosts.append((batch, osh, sdev.bits(db.q), sdev.bits(db.k_new), sdev.bits(db.v_new), sdev.bits(db.k_pool),
+                      sdev.bits(db.v_pool)))
+        del db
+    torch.cuda.empty_cache()
+    steps, tokens, dt = 0, 0, 0.0
+    while dt < seconds_budget and steps < 2000:
+        batch, osh, q, kn, vn, kp, vp = hosts[steps % len(hosts)]
+        rows = np.arange(batch.n_tok, dtype=np.int64)
+        t0 = time.perf_counter()
+        oracle.kv_append(osh, kn, vn, kp, vp, batch.cu_seqlens_q, batch.context_lens, batch.block_tables)
+        oracle.attention(osh, q, kp, vp, batch.cu_seqlens_q, batch.context_lens, batch.block_tables,
+                         batch.softmax_scale, rows=rows, n_threads=cores)
+        dt += time.perf_counter() - t0
+        steps += 1
+        tokens += batch.n_tok
+    return {"value": tokens / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt, "steps": steps,
+            "sample": f"{steps} whole C2 steps (kv_append + attention of all 2048 rows each, r cycled 0.0..1.0 as in the "
+                      f"timed region; inputs resident in host memory), fp64 oracle, {cores} threads, {dt:.1f} s of CPU work"}
 
 
 def run_ours(args):
@@ -260,18 +285,12 @@ def run_ours(args):
         attn_sec = [a.elapsed_time(b) * 1e-3 for a, b in kev]
         attn_bytes = [preps[i % len(preps)].batch.algorithmic_bytes() for i in range(K)]
         attn_roof = [_roof_seconds(preps[i % len(preps)].batch, peaks)[0] for i in range(K)]
-        if world > 1:
-            t = torch.tensor([sec], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            sec = float(t.item())
+        sec = max_over_ranks(sec, dev)
 
         # ---------------- e2e: host buffers in, host result out, through the public binding
         e2e = _e2e(preps, K, W, dev)
-        if world > 1:
-            t = torch.tensor([e2e["seconds"]], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e["seconds"] = float(t.item())
-        e2e_value = world * tokens / e2e.pop("seconds")
+        e2e["seconds"] = max_over_ranks(e2e["seconds"], dev)
+        e2e_value = job_throughput(tokens, e2e.pop("seconds"), world)
 
         sweep, fits, roofline, extra, cpu = [], [], None, {}, None
         if rank == 0:
@@ -304,7 +323,7 @@ def run_ours(args):
     clocks = sampler.summary()
 
     if rank == 0:
-        line = {"metric": METRIC, "value": world * tokens / sec, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        line = {"metric": METRIC, "value": job_throughput(tokens, sec, world), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": sec / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "bf16", "data": "synthetic",
                 "config": {"workload": "C2 Qwen3-4B-shaped attention layer (32/8/128, block 16), n_tok=2048/step, "
