@@ -129,6 +129,52 @@ __device__ __forceinline__ float fast_exp2(float x) {
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+// ---------------------------------------------------------------- packed fp32x2 arithmetic (sm_100: FFMA2 / FADD2)
+__device__ __forceinline__ uint64_t pack_f2(float lo, float hi) {
+    uint64_t v;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(lo), "f"(hi));
+    return v;
+}
+__device__ __forceinline__ void unpack_f2(uint64_t v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ uint64_t fadd2_rm(uint64_t a, uint64_t b) {     // round toward -inf
+    uint64_t d;
+    asm("add.rm.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ uint64_t fsub2(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+// 2^x for a pair, x in [-127, 127], on the FMA pipe instead of the 16-lane MUFU: floor by a round-down magic add,
+// degree-3 minimax polynomial of 2^f on [0,1) (max relative error 8.6e-5, below the bf16 rounding of P), exponent
+// inserted with an integer add.  The prefill softmax is MUFU-bound; a share of its exponentials
+// goes through here so that the MUFU and FMA pipes split the work.
+__device__ __forceinline__ void exp2_poly2(uint64_t x, float& p0, float& p1) {
+    const uint64_t xr = fadd2_rm(x, pack_f2(12582912.f, 12582912.f));        // 1.5·2^23 + floor(x)
+    const uint64_t fl = fadd2(xr, pack_f2(-12582912.f, -12582912.f));         // floor(x), exact
+    const uint64_t f = fsub2(x, fl);                                          // x - floor(x) in [0, 1)
+    uint64_t p = ffma2(f, pack_f2(0.0770670548081398f, 0.0770670548081398f), pack_f2(0.22764497995376587f, 0.22764497995376587f));
+    p = ffma2(p, f, pack_f2(0.6951168179512024f, 0.6951168179512024f));
+    p = ffma2(p, f, pack_f2(1.f, 1.f));
+    float q0, q1, r0, r1;
+    unpack_f2(p, q0, q1);
+    unpack_f2(xr, r0, r1);
+    p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(r0) << 23));
+    p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(r1) << 23));
+}
 __device__ __forceinline__ float fast_rcp(float x) {
     float y;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -168,6 +214,33 @@ __device__ __forceinline__ void umma_ts(uint32_t tmem_d, uint32_t tmem_a, uint64
         "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
         ::"r"(tmem_d), "r"(tmem_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
         : "memory");
+}
+// Elected-lane forms for warp-uniform issue code: every lane executes the surrounding control flow and address
+// arithmetic (which therefore stays in the uniform datapath: UTCHMMA/UTMALDG take uniform-register operands), and
+// only the lane chosen by elect.sync issues the instruction.  Call with all 32 lanes converged.
+__device__ __forceinline__ uint32_t elect_one() {
+    uint32_t pred = 0;
+    asm volatile(
+        "{\n\t.reg .pred px;\n\t"
+        "elect.sync _|px, 0xffffffff;\n\t"
+        "@px mov.s32 %0, 1;\n\t}"
+        : "+r"(pred));
+    return pred;
+}
+__device__ __forceinline__ void umma_ss_p(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
+    if (elect_one()) umma_ss(tmem_d, desc_a, desc_b, idesc, accumulate);
+}
+__device__ __forceinline__ void umma_ts_p(uint32_t tmem_d, uint32_t tmem_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
+    if (elect_one()) umma_ts(tmem_d, tmem_a, desc_b, idesc, accumulate);
+}
+__device__ __forceinline__ void umma_commit_p(uint32_t bar) {
+    if (elect_one()) umma_commit(bar);
+}
+__device__ __forceinline__ void tma_load_4d_p(uint32_t dst, const CUtensorMap* m, uint32_t bar, int c0, int c1, int c2, int c3) {
+    if (elect_one()) tma_load_4d(dst, m, bar, c0, c1, c2, c3);
+}
+__device__ __forceinline__ void mbar_expect_tx_p(uint32_t bar, uint32_t bytes) {
+    if (elect_one()) mbar_expect_tx(bar, bytes);
 }
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
     asm volatile(

@@ -29,6 +29,11 @@
 namespace pa {
 
 constexpr int kAttnThreads = 384;   // 12 warps: control warpgroup + two softmax warpgroups
+// pairs (of the 16 pairs of a 32-column chunk) whose exponentials run on the FMA pipe (exp2_poly2) instead of MUFU
+#ifndef PA_POLY_MASK
+#define PA_POLY_MASK 0x0000u
+#endif
+constexpr uint32_t kPolyMask = PA_POLY_MASK;
 
 template <int D, bool kPinTmem>
 struct PrefillCfg {
@@ -78,7 +83,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                              uint8_t* tiles, PrefillCtrl* ctrl, int first_unit) {
     using Cfg = PrefillCfg<D, kPinTmem>;
     constexpr int NQ = Cfg::NQ, KT = Cfg::KT, ST = Cfg::kStages;
-    const int warp = threadIdx.x >> 5, lane = lane_id();
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = lane_id();
     const PlanView& pl = p.plan;
     const uint32_t tiles_u32 = smem_u32(tiles);
 
@@ -107,7 +112,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
             ctrl->unit[it & 1] = u;
         }
         __syncthreads();
-        unit = ctrl->unit[it & 1];
+        unit = __shfl_sync(0xffffffffu, ctrl->unit[it & 1], 0);     // the same for all threads; the shuffle lets the compiler know
         if (unit >= pl.n_units) break;
 
         const int per_tile = p.Hkv * pl.head_groups;
@@ -130,9 +135,15 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                         tma_load_3d(tiles_u32 + Cfg::kOffQ + t * Cfg::kQBytes + c * (kQTile * 128), tmQ, smem_u32(&ctrl->q_full),
                                     c * 64, h_first + t, tile.row0 + tile.q_begin);
             }
+            // K/V tiles: every lane runs the same loop on warp-uniform values (lane-0 shuffles make that provable, so
+            // the box addresses stay in the uniform datapath); lane b fetches the id of block b, the ids are broadcast
+            // one by one and the elected lane issues the boxes.
+            const uint32_t ring_base = tiles_u32 + Cfg::kOffRing;
+            const int nkv_u = __shfl_sync(0xffffffffu, n_kv, 0), kvt_u = __shfl_sync(0xffffffffu, kv_total, 0);
+            const int kvh_u = __shfl_sync(0xffffffffu, kvh, 0);
             const int32_t* bt = p.block_tables + (int64_t)tile.seq * p.max_blocks_per_seq;
-            for (int j = 0; j < n_kv; ++j) {
-                const int keys = min(KT, kv_total - j * KT);
+            for (int j = 0; j < nkv_u; ++j) {
+                const int keys = min(KT, kvt_u - j * KT);
                 const int nb = (keys + kBlock - 1) / kBlock;
                 const int blk = (lane < nb) ? __ldg(bt + j * Cfg::kBlocksPerTile + lane) : 0;
 #pragma unroll
@@ -140,54 +151,76 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                     const uint32_t stage = ring % ST, ph = (ring / ST) & 1u;
                     const uint32_t full = smem_u32(&ctrl->kv_full[stage]);
                     mbar_wait(smem_u32(&ctrl->kv_empty[stage]), ph ^ 1u);
-                    if (lane == 0) mbar_expect_tx(full, nb * (kBlock * D * 2));
-                    __syncwarp();
-                    if (lane < nb) {
-                        const uint32_t dst = tiles_u32 + Cfg::kOffRing + stage * Cfg::kStageBytes + lane * 2048;
+                    mbar_expect_tx_p(full, nb * (kBlock * D * 2));
+                    const uint32_t dst = ring_base + stage * Cfg::kStageBytes;
+                    if (nb == Cfg::kBlocksPerTile) {
 #pragma unroll
-                        for (int c = 0; c < D / 64; ++c)
-                            tma_load_4d(dst + c * (KT * 128), isV ? tmV : tmK, full, c * 64, 0, kvh, blk);
+                        for (int bb = 0; bb < Cfg::kBlocksPerTile; ++bb) {
+                            const int id = __shfl_sync(0xffffffffu, blk, bb);
+#pragma unroll
+                            for (int c = 0; c < D / 64; ++c)
+                                tma_load_4d_p(dst + bb * 2048 + c * (KT * 128), isV ? tmV : tmK, full, c * 64, 0, kvh_u, id);
+                        }
+                    } else {
+                        for (int bb = 0; bb < nb; ++bb) {
+                            const int id = __shfl_sync(0xffffffffu, blk, bb);
+#pragma unroll
+                            for (int c = 0; c < D / 64; ++c)
+                                tma_load_4d_p(dst + bb * 2048 + c * (KT * 128), isV ? tmV : tmK, full, c * 64, 0, kvh_u, id);
+                        }
                     }
                     ++ring;
                 }
             }
         } else if (warp == 1) {
             // ======================================================== MMA issuer
+            // Warp-uniform control flow; tcgen05.mma / tcgen05.commit are predicated on the elected lane and their
+            // descriptors advance by compile-time constants, so issuing an MMA costs a few uniform instructions
+            // (the issue rate of this one warp bounds the tensor pipe: 32 MMAs per KV tile).
             constexpr uint32_t idescS = umma_idesc_bf16(128, KT, 0);
             constexpr uint32_t idescO = umma_idesc_bf16(128, D, 1);
-            const uint32_t q_base = tiles_u32 + Cfg::kOffQ;
+            const uint32_t tm = __shfl_sync(0xffffffffu, tmem, 0);
+            const uint32_t sbase = tiles_u32;
+            const int nkv_u = __shfl_sync(0xffffffffu, n_kv, 0), kvt_u = __shfl_sync(0xffffffffu, kv_total, 0);
+            const int kvl_u = __shfl_sync(0xffffffffu, tile.kv_len, 0), nact_u = __shfl_sync(0xffffffffu, nact, 0);
             auto issue_S = [&](int t, uint32_t kstage) {      // S_t = Q_t · K^T   (D/16 k-steps)
-                if (lane == 0) {
-                    const uint32_t qa = q_base + t * Cfg::kQBytes;
-                    const uint32_t kb = tiles_u32 + Cfg::kOffRing + kstage * Cfg::kStageBytes;
+                const uint64_t da0 = umma_desc_sw128(sbase + Cfg::kOffQ + t * Cfg::kQBytes, 16, 1024);
+                const uint64_t db0 = umma_desc_sw128(sbase + Cfg::kOffRing + kstage * Cfg::kStageBytes, 16, 1024);
 #pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks) {
-                        const uint64_t da = umma_desc_sw128(qa + (ks >> 2) * (kQTile * 128) + (ks & 3) * 32, 16, 1024);
-                        const uint64_t db = umma_desc_sw128(kb + (ks >> 2) * (KT * 128) + (ks & 3) * 32, 16, 1024);
-                        umma_ss(tmem + Cfg::kColS + t * KT, da, db, idescS, ks > 0);
-                    }
-                    umma_commit(smem_u32(&ctrl->s_full[t]));
+                for (int ks = 0; ks < D / 16; ++ks) {
+                    const uint32_t oa = (uint32_t)(((ks >> 2) * (kQTile * 128) + (ks & 3) * 32) >> 4);
+                    const uint32_t ob = (uint32_t)(((ks >> 2) * (KT * 128) + (ks & 3) * 32) >> 4);
+                    umma_ss_p(tm + Cfg::kColS + t * KT, da0 + oa, db0 + ob, idescS, ks > 0);
                 }
-                __syncwarp();
+                umma_commit_p(smem_u32(&ctrl->s_full[t]));
+            };
+            auto issue_PV = [&](int t, uint32_t vb, int ks, uint32_t acc) {   // O_t += P_t[:, 16 ks..] · V[16 ks.., :]
+                const uint64_t db = umma_desc_sw128(vb, KT * 128, 1024) + (uint64_t)(ks * (2048 >> 4));
+                if constexpr (kPinTmem) {
+                    umma_ts_p(tm + Cfg::kColO + t * D, tm + Cfg::kColS + t * KT + ks * 8, db, idescO, acc);
+                } else {
+                    const uint64_t da = umma_desc_sw128(sbase + Cfg::kOffP + t * Cfg::kPBytes, 16, 1024) +
+                                        (uint64_t)(((ks >> 2) * (kQTile * 128) + (ks & 3) * 32) >> 4);
+                    umma_ss_p(tm + Cfg::kColO + t * D, da, db, idescO, acc);
+                }
             };
             mbar_wait(smem_u32(&ctrl->q_full), n_unit & 1u);
             {   // S(0)
                 const uint32_t stage = ring % ST, ph = (ring / ST) & 1u;
                 mbar_wait(smem_u32(&ctrl->kv_full[stage]), ph);
                 tc_fence_after();
-                for (int t = 0; t < nact; ++t) issue_S(t, stage);
-                if (lane == 0) umma_commit(smem_u32(&ctrl->kv_empty[stage]));
-                __syncwarp();
+                for (int t = 0; t < nact_u; ++t) issue_S(t, stage);
+                umma_commit_p(smem_u32(&ctrl->kv_empty[stage]));
                 ++ring;
             }
-            for (int j = 0; j < n_kv; ++j) {
+            for (int j = 0; j < nkv_u; ++j) {
                 const uint32_t sv = ring % ST, phv = (ring / ST) & 1u;
                 ++ring;
                 mbar_wait(smem_u32(&ctrl->kv_full[sv]), phv);
-                const int keys = min(KT, kv_total - j * KT);
+                const int keys = min(KT, kvt_u - j * KT);
                 const int nks = (keys + kBlock - 1) / kBlock;            // PV k-steps = loaded blocks
-                const uint32_t vb = tiles_u32 + Cfg::kOffRing + sv * Cfg::kStageBytes;
-                const int first_dead = tile.kv_len - j * KT;             // rows >= this hold no token (R8)
+                const uint32_t vb = sbase + Cfg::kOffRing + sv * Cfg::kStageBytes;
+                const int first_dead = kvl_u - j * KT;                   // rows >= this hold no token (R8)
                 if (first_dead < nks * kBlock) {
                     // zero them: masked P is exactly 0, but 0 x NaN (sentinel / garbage) would poison O
                     const int nrows = nks * kBlock - first_dead;
@@ -200,26 +233,18 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                     __syncwarp();
                 }
                 uint32_t sk = 0;
-                for (int t = 0; t < nact; ++t) {
+                for (int t = 0; t < nact_u; ++t) {
                     mbar_wait(smem_u32(&ctrl->p_full[t]), t == 0 ? pph0 : pph1);
                     tc_fence_after();
-                    if (lane == 0) {
-                        for (int ks = 0; ks < nks; ++ks) {
-                            const uint64_t db = umma_desc_sw128(vb + ks * 2048, KT * 128, 1024);
-                            const uint32_t acc = (j > 0 || ks > 0) ? 1u : 0u;
-                            if constexpr (kPinTmem) {
-                                umma_ts(tmem + Cfg::kColO + t * D, tmem + Cfg::kColS + t * KT + ks * 8, db, idescO, acc);
-                            } else {
-                                const uint32_t pa_ = tiles_u32 + Cfg::kOffP + t * Cfg::kPBytes;
-                                const uint64_t da = umma_desc_sw128(pa_ + (ks >> 2) * (kQTile * 128) + (ks & 3) * 32, 16, 1024);
-                                umma_ss(tmem + Cfg::kColO + t * D, da, db, idescO, acc);
-                            }
-                        }
-                        if (t == nact - 1) umma_commit(smem_u32(&ctrl->kv_empty[sv]));
-                        if (j == n_kv - 1) umma_commit(smem_u32(&ctrl->o_full[t]));
+                    if (nks == KT / kBlock) {
+#pragma unroll
+                        for (int ks = 0; ks < KT / kBlock; ++ks) issue_PV(t, vb, ks, (j > 0 || ks > 0) ? 1u : 0u);
+                    } else {
+                        for (int ks = 0; ks < nks; ++ks) issue_PV(t, vb, ks, (j > 0 || ks > 0) ? 1u : 0u);
                     }
-                    __syncwarp();
-                    if (j + 1 < n_kv) {
+                    if (t == nact_u - 1) umma_commit_p(smem_u32(&ctrl->kv_empty[sv]));
+                    if (j == nkv_u - 1) umma_commit_p(smem_u32(&ctrl->o_full[t]));
+                    if (j + 1 < nkv_u) {
                         if (t == 0) {
                             sk = ring % ST;
                             const uint32_t phk = (ring / ST) & 1u;
@@ -228,17 +253,13 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                             tc_fence_after();
                         }
                         issue_S(t, sk);
-                        if (t == nact - 1) {
-                            if (lane == 0) umma_commit(smem_u32(&ctrl->kv_empty[sk]));
-                            __syncwarp();
-                        }
+                        if (t == nact_u - 1) umma_commit_p(smem_u32(&ctrl->kv_empty[sk]));
                     }
                 }
                 pph0 ^= 1u;
-                if (nact > 1) pph1 ^= 1u;
+                if (nact_u > 1) pph1 ^= 1u;
             }
-            if (lane == 0) umma_commit(smem_u32(&ctrl->q_empty));
-            __syncwarp();
+            umma_commit_p(smem_u32(&ctrl->q_empty));
         } else if (warp >= 4) {
             // ======================================================== softmax + correction + epilogue
             const int t = (warp - 4) >> 2;
@@ -250,37 +271,21 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                 const int limit = tile.ctx + tile.q_begin + row;        // keys 0 .. limit are visible (R3)
                 const float sl = p.scale_log2;
                 const float NEG_INF = -INFINITY;
-                float m_ref = NEG_INF, l = 0.f;
+                // m_ref: the reference max the exponentials of a tile are taken against; m_run: max of all scores seen.
+                // Only the first tile needs its own max before exponentiating (two passes over S); later tiles use the
+                // reference left by their predecessors and fold the max into the same pass, so S is read from TMEM
+                // once.  The reference is moved (l and the O row rescaled) at the start of a tile, and only when the
+                // running max outgrew it by more than 2^8; within a tile P may therefore exceed 1 by the growth of
+                // that one tile, which floating point absorbs (P <= 2^64 is left alone; beyond it the row is fixed up
+                // exactly, see below).
+                float m_ref = NEG_INF, m_run = NEG_INF, l = 0.f;
                 for (int j = 0; j < n_kv; ++j) {
                     mbar_wait(smem_u32(&ctrl->s_full[t]), sph);
                     sph ^= 1u;
                     tc_fence_after();
                     const int kbase = j * KT;
                     const bool need_mask = kbase + KT - 1 > tile.ctx + tile.q_begin;
-                    // ---- pass 1: row maximum of the raw scores
-                    float mx = NEG_INF;
-#pragma unroll
-                    for (int c = 0; c < KT / 32; ++c) {
-                        uint32_t r[32];
-                        tmem_ld32(tS + c * 32, r);
-                        tmem_wait_ld();
-                        if (need_mask) {
-#pragma unroll
-                            for (int i = 0; i < 32; ++i)
-                                mx = fmaxf(mx, (kbase + c * 32 + i <= limit) ? __uint_as_float(r[i]) : NEG_INF);
-                        } else {
-#pragma unroll
-                            for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(r[i]));
-                        }
-                    }
-                    const float m_new = fmaxf(m_ref, mx);
-                    if (j == 0) {
-                        m_ref = m_new;
-                    } else if (__any_sync(0xffffffffu, (m_new - m_ref) * sl > 8.f)) {
-                        // lazy correction: rescale l and the O row only when the max moved by > 2^8
-                        const float alpha = fast_exp2((m_ref - m_new) * sl);
-                        l *= alpha;
-                        m_ref = m_new;
+                    auto rescale_o = [&](float alpha) {
 #pragma unroll
                         for (int c = 0; c < D / 32; ++c) {
                             uint32_t r[32];
@@ -291,14 +296,45 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                             tmem_st32(tO + c * 32, r);
                         }
                         tmem_wait_st();
+                    };
+                    if (j == 0) {
+                        // ---- first tile: row maximum of the raw scores
+                        float mx = NEG_INF;
+#pragma unroll
+                        for (int c = 0; c < KT / 32; ++c) {
+                            uint32_t r[32];
+                            tmem_ld32(tS + c * 32, r);
+                            tmem_wait_ld();
+                            if (need_mask) {
+#pragma unroll
+                                for (int i = 0; i < 32; ++i)
+                                    mx = fmaxf(mx, (kbase + c * 32 + i <= limit) ? __uint_as_float(r[i]) : NEG_INF);
+                            } else {
+#pragma unroll
+                                for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(r[i]));
+                            }
+                        }
+                        m_ref = m_run = mx;
+                    } else if (__any_sync(0xffffffffu, (m_run - m_ref) * sl > 8.f)) {
+                        // lazy correction: O holds the tiles before this one (their PV MMAs completed before s_full)
+                        const float alpha = fast_exp2((m_ref - m_run) * sl);
+                        l *= alpha;
+                        m_ref = m_run;
+                        rescale_o(alpha);
                     }
                     const float neg = -m_ref * sl;
-                    // ---- pass 2: P = exp2(s*sl - m_ref*sl) -> bf16 (TMEM over S, or swizzled shared memory)
+                    // ---- P = exp2(s*sl - m_ref*sl) -> bf16 (TMEM over S, or swizzled shared memory) and the tile max,
+                    // one pass, packed f32x2 math; the TMEM load of chunk c+1 is in flight while chunk c is processed.
+                    const uint64_t sl2 = pack_f2(sl, sl), neg2 = pack_f2(neg, neg);
+                    uint64_t lsum = pack_f2(0.f, 0.f);
+                    float mx = NEG_INF;
+                    uint32_t rbuf[2][32];
+                    tmem_ld32(tS, rbuf[0]);
 #pragma unroll
                     for (int c = 0; c < KT / 32; ++c) {
-                        uint32_t r[32];
-                        tmem_ld32(tS + c * 32, r);
+                        uint32_t (&r)[32] = rbuf[c & 1];
                         tmem_wait_ld();
+                        if (c + 1 < KT / 32) tmem_ld32(tS + (c + 1) * 32, rbuf[(c + 1) & 1]);
                         uint32_t pk[16];
 #pragma unroll
                         for (int i = 0; i < 32; i += 2) {
@@ -307,8 +343,17 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                                 if (kbase + c * 32 + i > limit) s0 = NEG_INF;
                                 if (kbase + c * 32 + i + 1 > limit) s1 = NEG_INF;
                             }
-                            const float p0 = fast_exp2(fmaf(s0, sl, neg)), p1 = fast_exp2(fmaf(s1, sl, neg));
-                            l += p0 + p1;
+                            mx = fmaxf(mx, fmaxf(s0, s1));
+                            const uint64_t x = ffma2(pack_f2(s0, s1), sl2, neg2);
+                            float x0, x1, p0, p1;
+                            unpack_f2(x, x0, x1);
+                            if ((kPolyMask >> (i >> 1)) & 1u) {
+                                exp2_poly2(pack_f2(fmaxf(x0, -127.f), fmaxf(x1, -127.f)), p0, p1);
+                            } else {
+                                p0 = fast_exp2(x0);
+                                p1 = fast_exp2(x1);
+                            }
+                            lsum = fadd2(lsum, pack_f2(p0, p1));
                             pk[i >> 1] = pack_bf16x2(p0, p1);
                         }
                         if constexpr (kPinTmem) {
@@ -324,6 +369,45 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                                              : "memory");
                             }
                         }
+                    }
+                    {
+                        float la, lb;
+                        unpack_f2(lsum, la, lb);
+                        l += la + lb;
+                    }
+                    m_run = fmaxf(m_run, mx);
+                    if (j > 0 && __any_sync(0xffffffffu, (mx - m_ref) * sl > 64.f)) {
+                        // rare: this tile outgrew the reference by more than 2^64.  Its P (finite up to 2^127) is scaled
+                        // down by the exact power of two alpha, together with l and the O row, and the reference moves.
+                        const bool mine = (mx - m_ref) * sl > 64.f;
+                        const float alpha = mine ? fast_exp2(floorf((m_ref - mx) * sl)) : 1.f;
+                        if (mine) m_ref += -floorf((m_ref - mx) * sl) / sl;
+                        l *= alpha;
+                        if constexpr (kPinTmem) {
+                            tmem_wait_st();
+#pragma unroll
+                            for (int c = 0; c < KT / 64; ++c) {
+                                uint32_t r[32];
+                                tmem_ld32(tS + c * 32, r);
+                                tmem_wait_ld();
+#pragma unroll
+                                for (int i = 0; i < 32; ++i)
+                                    r[i] = pack_bf16x2(__uint_as_float(r[i] << 16) * alpha, __uint_as_float(r[i] & 0xffff0000u) * alpha);
+                                tmem_st32(tS + c * 32, r);
+                            }
+                        } else {
+                            const uint32_t pbase = tiles_u32 + Cfg::kOffP + t * Cfg::kPBytes;
+                            for (int cc = 0; cc < KT / 8; ++cc) {
+                                const uint32_t addr = pbase + (cc >> 3) * (kQTile * 128) + swz128(row, cc & 7);
+                                uint32_t v[4];
+                                asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(addr) : "memory");
+#pragma unroll
+                                for (int i = 0; i < 4; ++i)
+                                    v[i] = pack_bf16x2(__uint_as_float(v[i] << 16) * alpha, __uint_as_float(v[i] & 0xffff0000u) * alpha);
+                                asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]) : "memory");
+                            }
+                        }
+                        rescale_o(alpha);
                     }
                     if constexpr (kPinTmem) tmem_wait_st();
                     else fence_proxy_async();

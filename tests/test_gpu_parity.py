@@ -107,6 +107,36 @@ def test_split_kv_groups_merge_in_launch():
     gc.check_close(sdev.bits(d["out"]), ref, "split")
 
 
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("shape_name", ["QWEN3_4B", "GEMMA3_1B"])
+def test_prefill_running_max_growth(shape_name, mode, monkeypatch):
+    """Scores that grow along the keys: the prefill softmax exponentiates a tile against the reference max left by
+    earlier tiles, so the three regimes must all match the oracle: growth below 2^8 (reference kept),
+    above 2^8 (lazy rescale of l and O at the next tile) and above 2^64 within one tile (exact power-of-two fix-up)."""
+    monkeypatch.setenv("PA_PREFILL_MODE", str(mode))
+    W = workloads
+    shape = getattr(W, shape_name)
+    ctx, q_len = 500, 300
+    batch = W.make_batch("growth", shape, 211, [1, q_len], [40, ctx], 1)
+    inp = helpers.host_inputs(batch)
+    gain = {0: 0.0, 1: 12.0, 2: 12.0, 3: 120.0, 4: 120.0, 5: 1.0}      # per 128 keys; the rest keeps its N(0,1) draw
+    b = shape.block_size
+    bits = lambda v: gen.f32_to_bf16(np.array([v], dtype=np.float32))[0]
+    row0 = int(batch.cu_seqlens_q[1])
+    inp["q"][row0:row0 + q_len, :, 0] = bits(8.0)
+    for t in range(ctx + q_len):
+        if t // 128 not in gain:
+            continue
+        v = bits(gain[t // 128])
+        if t < ctx:
+            inp["k_pool"][int(batch.block_tables[1, t // b]), :, t % b, 0] = v
+        else:
+            inp["k_new"][row0 + t - ctx, :, 0] = v
+    d = gc.run_gpu(batch, inp)
+    ref, _, _ = gc.run_oracle(batch, inp)
+    gc.check_close(sdev.bits(d["out"]), ref, f"growth/{shape_name}/mode{mode}")
+
+
 def test_repeated_launches_are_deterministic_and_reset_state():
     batch = _small_case("ragged-g4-d128")
     inp = helpers.host_inputs(batch)
