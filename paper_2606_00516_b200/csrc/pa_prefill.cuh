@@ -83,7 +83,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                              uint8_t* tiles, PrefillCtrl* ctrl, int first_unit) {
     using Cfg = PrefillCfg<D, kPinTmem>;
     constexpr int NQ = Cfg::NQ, KT = Cfg::KT, ST = Cfg::kStages;
-    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = lane_id();
+    const int warp = (int)__reduce_max_sync(0xffffffffu, threadIdx.x >> 5), lane = lane_id();
     const PlanView& pl = p.plan;
     const uint32_t tiles_u32 = smem_u32(tiles);
 
@@ -112,7 +112,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
             ctrl->unit[it & 1] = u;
         }
         __syncthreads();
-        unit = __shfl_sync(0xffffffffu, ctrl->unit[it & 1], 0);     // the same for all threads; the shuffle lets the compiler know
+        unit = __reduce_max_sync(0xffffffffu, ctrl->unit[it & 1]);   // the same for all threads; a warp reduction lands in a uniform register, so the compiler knows it
         if (unit >= pl.n_units) break;
 
         const int per_tile = p.Hkv * pl.head_groups;
@@ -139,36 +139,34 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
             // the box addresses stay in the uniform datapath); lane b fetches the id of block b, the ids are broadcast
             // one by one and the elected lane issues the boxes.
             const uint32_t ring_base = tiles_u32 + Cfg::kOffRing;
-            const int nkv_u = __shfl_sync(0xffffffffu, n_kv, 0), kvt_u = __shfl_sync(0xffffffffu, kv_total, 0);
-            const int kvh_u = __shfl_sync(0xffffffffu, kvh, 0);
+            const int nkv_u = __reduce_max_sync(0xffffffffu, n_kv), kvt_u = __reduce_max_sync(0xffffffffu, kv_total);
+            const int kvh_u = __reduce_max_sync(0xffffffffu, kvh);
             const int32_t* bt = p.block_tables + (int64_t)tile.seq * p.max_blocks_per_seq;
             for (int j = 0; j < nkv_u; ++j) {
                 const int keys = min(KT, kvt_u - j * KT);
                 const int nb = (keys + kBlock - 1) / kBlock;
                 const int blk = (lane < nb) ? __ldg(bt + j * Cfg::kBlocksPerTile + lane) : 0;
+                int ids[Cfg::kBlocksPerTile];
+#pragma unroll
+                for (int bb = 0; bb < Cfg::kBlocksPerTile; ++bb) ids[bb] = __shfl_sync(0xffffffffu, blk, bb);
 #pragma unroll
                 for (int isV = 0; isV < 2; ++isV) {
                     const uint32_t stage = ring % ST, ph = (ring / ST) & 1u;
                     const uint32_t full = smem_u32(&ctrl->kv_full[stage]);
                     mbar_wait(smem_u32(&ctrl->kv_empty[stage]), ph ^ 1u);
-                    mbar_expect_tx_p(full, nb * (kBlock * D * 2));
-                    const uint32_t dst = ring_base + stage * Cfg::kStageBytes;
-                    if (nb == Cfg::kBlocksPerTile) {
+                    if (elect_one()) {
+                        mbar_expect_tx(full, nb * (kBlock * D * 2));
+                        const uint32_t dst = ring_base + stage * Cfg::kStageBytes;
 #pragma unroll
                         for (int bb = 0; bb < Cfg::kBlocksPerTile; ++bb) {
-                            const int id = __shfl_sync(0xffffffffu, blk, bb);
+                            if (bb < nb) {
 #pragma unroll
-                            for (int c = 0; c < D / 64; ++c)
-                                tma_load_4d_p(dst + bb * 2048 + c * (KT * 128), isV ? tmV : tmK, full, c * 64, 0, kvh_u, id);
-                        }
-                    } else {
-                        for (int bb = 0; bb < nb; ++bb) {
-                            const int id = __shfl_sync(0xffffffffu, blk, bb);
-#pragma unroll
-                            for (int c = 0; c < D / 64; ++c)
-                                tma_load_4d_p(dst + bb * 2048 + c * (KT * 128), isV ? tmV : tmK, full, c * 64, 0, kvh_u, id);
+                                for (int c = 0; c < D / 64; ++c)
+                                    tma_load_4d(dst + bb * 2048 + c * (KT * 128), isV ? tmV : tmK, full, c * 64, 0, kvh_u, ids[bb]);
+                            }
                         }
                     }
+                    __syncwarp();
                     ++ring;
                 }
             }
@@ -179,29 +177,32 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
             // (the issue rate of this one warp bounds the tensor pipe: 32 MMAs per KV tile).
             constexpr uint32_t idescS = umma_idesc_bf16(128, KT, 0);
             constexpr uint32_t idescO = umma_idesc_bf16(128, D, 1);
-            const uint32_t tm = __shfl_sync(0xffffffffu, tmem, 0);
+            const uint32_t tm = __reduce_max_sync(0xffffffffu, tmem);
             const uint32_t sbase = tiles_u32;
-            const int nkv_u = __shfl_sync(0xffffffffu, n_kv, 0), kvt_u = __shfl_sync(0xffffffffu, kv_total, 0);
-            const int kvl_u = __shfl_sync(0xffffffffu, tile.kv_len, 0), nact_u = __shfl_sync(0xffffffffu, nact, 0);
+            const int nkv_u = __reduce_max_sync(0xffffffffu, n_kv), kvt_u = __reduce_max_sync(0xffffffffu, kv_total);
+            const int kvl_u = __reduce_max_sync(0xffffffffu, tile.kv_len), nact_u = __reduce_max_sync(0xffffffffu, nact);
             auto issue_S = [&](int t, uint32_t kstage) {      // S_t = Q_t · K^T   (D/16 k-steps)
-                const uint64_t da0 = umma_desc_sw128(sbase + Cfg::kOffQ + t * Cfg::kQBytes, 16, 1024);
-                const uint64_t db0 = umma_desc_sw128(sbase + Cfg::kOffRing + kstage * Cfg::kStageBytes, 16, 1024);
+                if (elect_one()) {
+                    const uint64_t da0 = umma_desc_sw128(sbase + Cfg::kOffQ + t * Cfg::kQBytes, 16, 1024);
+                    const uint64_t db0 = umma_desc_sw128(sbase + Cfg::kOffRing + kstage * Cfg::kStageBytes, 16, 1024);
 #pragma unroll
-                for (int ks = 0; ks < D / 16; ++ks) {
-                    const uint32_t oa = (uint32_t)(((ks >> 2) * (kQTile * 128) + (ks & 3) * 32) >> 4);
-                    const uint32_t ob = (uint32_t)(((ks >> 2) * (KT * 128) + (ks & 3) * 32) >> 4);
-                    umma_ss_p(tm + Cfg::kColS + t * KT, da0 + oa, db0 + ob, idescS, ks > 0);
+                    for (int ks = 0; ks < D / 16; ++ks) {
+                        const uint32_t oa = (uint32_t)(((ks >> 2) * (kQTile * 128) + (ks & 3) * 32) >> 4);
+                        const uint32_t ob = (uint32_t)(((ks >> 2) * (KT * 128) + (ks & 3) * 32) >> 4);
+                        umma_ss(tm + Cfg::kColS + t * KT, da0 + oa, db0 + ob, idescS, ks > 0);
+                    }
+                    umma_commit(smem_u32(&ctrl->s_full[t]));
                 }
-                umma_commit_p(smem_u32(&ctrl->s_full[t]));
+                __syncwarp();
             };
             auto issue_PV = [&](int t, uint32_t vb, int ks, uint32_t acc) {   // O_t += P_t[:, 16 ks..] · V[16 ks.., :]
                 const uint64_t db = umma_desc_sw128(vb, KT * 128, 1024) + (uint64_t)(ks * (2048 >> 4));
                 if constexpr (kPinTmem) {
-                    umma_ts_p(tm + Cfg::kColO + t * D, tm + Cfg::kColS + t * KT + ks * 8, db, idescO, acc);
+                    umma_ts(tm + Cfg::kColO + t * D, tm + Cfg::kColS + t * KT + ks * 8, db, idescO, acc);
                 } else {
                     const uint64_t da = umma_desc_sw128(sbase + Cfg::kOffP + t * Cfg::kPBytes, 16, 1024) +
                                         (uint64_t)(((ks >> 2) * (kQTile * 128) + (ks & 3) * 32) >> 4);
-                    umma_ss_p(tm + Cfg::kColO + t * D, da, db, idescO, acc);
+                    umma_ss(tm + Cfg::kColO + t * D, da, db, idescO, acc);
                 }
             };
             mbar_wait(smem_u32(&ctrl->q_full), n_unit & 1u);
@@ -236,14 +237,17 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                 for (int t = 0; t < nact_u; ++t) {
                     mbar_wait(smem_u32(&ctrl->p_full[t]), t == 0 ? pph0 : pph1);
                     tc_fence_after();
-                    if (nks == KT / kBlock) {
+                    if (elect_one()) {
+                        if (nks == KT / kBlock) {
 #pragma unroll
-                        for (int ks = 0; ks < KT / kBlock; ++ks) issue_PV(t, vb, ks, (j > 0 || ks > 0) ? 1u : 0u);
-                    } else {
-                        for (int ks = 0; ks < nks; ++ks) issue_PV(t, vb, ks, (j > 0 || ks > 0) ? 1u : 0u);
+                            for (int ks = 0; ks < KT / kBlock; ++ks) issue_PV(t, vb, ks, (j > 0 || ks > 0) ? 1u : 0u);
+                        } else {
+                            for (int ks = 0; ks < nks; ++ks) issue_PV(t, vb, ks, (j > 0 || ks > 0) ? 1u : 0u);
+                        }
+                        if (t == nact_u - 1) umma_commit(smem_u32(&ctrl->kv_empty[sv]));
+                        if (j == nkv_u - 1) umma_commit(smem_u32(&ctrl->o_full[t]));
                     }
-                    if (t == nact_u - 1) umma_commit_p(smem_u32(&ctrl->kv_empty[sv]));
-                    if (j == nkv_u - 1) umma_commit_p(smem_u32(&ctrl->o_full[t]));
+                    __syncwarp();
                     if (j + 1 < nkv_u) {
                         if (t == 0) {
                             sk = ring % ST;
