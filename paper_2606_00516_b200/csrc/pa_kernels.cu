@@ -39,6 +39,9 @@ __global__ void __launch_bounds__(256) pa_kv_append_kernel(const int4* __restric
                                                            const int32_t* __restrict__ bt, int max_blocks_per_seq,
                                                            int Hkv, int n_seq, int n_tok) {
     constexpr int CPH = D / 8;  // 16-byte chunks per head row
+    // the attention launch that follows on the stream may bring its CTAs up (barrier init, descriptor prefetch)
+    // while the rows are copied; it reads the pool only after its grid-dependency wait
+    pdl_launch_dependents();
     const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (row >= n_tok) return;
     const int lane = lane_id();
@@ -147,6 +150,9 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
         fence_proxy_async();
     }
     __syncthreads();
+    // everything above touches only this CTA's shared memory and the kernel parameters; the pools, the plan and the
+    // queues are read below, after the preceding kernel of the stream (normally kv_append) has completed
+    pdl_grid_dependency_wait();
     const bool starts_prefill = (int)blockIdx.x < p.prefill_ctas;
     const int dec_rank = (int)blockIdx.x - p.prefill_ctas;       // rank among the initial decode CTAs
 #pragma unroll 1
@@ -209,13 +215,24 @@ cudaError_t launch_attention(const AttnLaunch& a, cudaStream_t stream, int* laun
         dim3 grid(grid_ctas), block(kAttnThreads);
         const CUtensorMap& tq = a.tmQ ? *a.tmQ : *a.tmK;    // unused when there are no prefill units
         const CUtensorMap& tqd = a.tmQd ? *a.tmQd : *a.tmK;  // unused when there are no decode bundles
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = grid;
+        cfg.blockDim = block;
+        cfg.dynamicSmemBytes = kAttnSmemBytes;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see pdl_grid_dependency_wait in the kernel
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
         if (a.sh.D == 128) {
-            if (a.p_in_tmem) pa_attention_kernel<128, true><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV, *a.tails);
-            else pa_attention_kernel<128, false><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV, *a.tails);
+            if (a.p_in_tmem) e = cudaLaunchKernelEx(&cfg, pa_attention_kernel<128, true>, p, tq, tqd, *a.tmK, *a.tmV, *a.tails);
+            else e = cudaLaunchKernelEx(&cfg, pa_attention_kernel<128, false>, p, tq, tqd, *a.tmK, *a.tmV, *a.tails);
         } else {
-            if (a.p_in_tmem) pa_attention_kernel<256, true><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV, *a.tails);
-            else pa_attention_kernel<256, false><<<grid, block, kAttnSmemBytes, stream>>>(p, tq, tqd, *a.tmK, *a.tmV, *a.tails);
+            if (a.p_in_tmem) e = cudaLaunchKernelEx(&cfg, pa_attention_kernel<256, true>, p, tq, tqd, *a.tmK, *a.tmV, *a.tails);
+            else e = cudaLaunchKernelEx(&cfg, pa_attention_kernel<256, false>, p, tq, tqd, *a.tmK, *a.tmV, *a.tails);
         }
+        if (e != cudaSuccess) return e;
         ++launches;
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
