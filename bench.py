@@ -7,15 +7,19 @@ Workload (N = 1): BASELINE.json configs[1] — Qwen3-4B-shaped attention layer (
 head_dim 128, block 16), n_tok = 2048 per step, decode sequences with ctx 16, 512-token prompts,
 decode ratio r swept 0.0 … 1.0 (Fig. 1 setup).  One *step* = kv_append +
 batch_attention (SURVEY §8(a) a3–a7, planned by a1) over one synthetic batch; the K timed steps cycle
-through the 11 r-batches (r_i = (i mod 11)/10), whose pools (11 × 0.5 GB) exceed L2, so every step
+through the 11 r-batches (r_i = (i mod 11)/10), whose pools (11 × 1 GB) exceed L2, so every step
 starts with cold inputs.  `value` = tokens / device time of those K steps (CUDA events, inputs resident
-in HBM).  `e2e` = the same through the public binding from pinned HOST buffers (H2D of q/k_new/v_new
+in HBM).  The same K steps are then repeated with an event pair around every attention launch: the live
+per-launch durations behind `roofline` (kept out of the headline loop: an event between kv_append and
+batch_attention would stop the attention CTAs from coming up under the append).
+`e2e` = the same through the public binding from pinned HOST buffers (H2D of q/k_new/v_new
 and the descriptors, pa_plan, kv_append, batch_attention, D2H of the output, per step).
 Also reported: per-r table (tokens/s, achieved GB/s, roofline fraction, alpha/beta/R² of
-T = alpha + beta·n_tok fitted through pa_timer_*), the bandwidth-bound C3 (Gemma-3-1B decode) line,
-with --extended C4 (Qwen3-8B mixed, n_tok 8192) and C5 (Qwen3-30B-A3B, 150 GB pool); the oracle timed on the
-host cores (cpu_baseline).  Multi-GPU: the path has no exchange step ("replicas only", DESIGN.md
-§8): each rank runs the same workload on its GPU, value = Σ tokens / max-over-ranks time.
+T = alpha + beta·n_tok fitted through pa_timer_*), kappa and the mixed-vs-exclusive comparison
+(SURVEY §8(f) N1/N3), the bandwidth-bound C3 (Gemma-3-1B decode) line, with --extended C4 (Qwen3-8B
+mixed, n_tok 8192) and C5 (Qwen3-30B-A3B, 150 GB pool); the oracle timed on the host cores
+(cpu_baseline).  Multi-GPU: the path has no exchange step ("replicas only"): each rank
+runs the same workload on its GPU, value = Σ tokens / max-over-ranks time.
 """
 from __future__ import annotations
 
@@ -39,8 +43,8 @@ FIT_NTOK = [512, 1024, 2048, 4096]          # DESIGN R18
 L2_FLUSH_BYTES = 512 << 20
 # dram__bytes_read.sum + dram__bytes_write.sum per pa_attention_kernel launch, mean over the 11 r-batches of C2,
 # from the ncu --set full capture summarised in profiles/ (None until that capture exists)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 95395840.0
-NCU_TRAFFIC_SOURCE = "profiles/r1e_c2_cycle.md (ncu --set full, 11 launches of one r-cycle)"
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 96015662.5
+NCU_TRAFFIC_SOURCE = "profiles/r1g_c2_cycle.md (ncu --set full, 11 launches of one r-cycle)"
 
 
 def _peaks():
@@ -163,6 +167,21 @@ def _roof_seconds(batch, peaks):
     return max(tb, tf), ("hbm" if tb >= tf else "tensor")
 
 
+class L2Flush:
+    """Cold AND clean L2 between repetitions: write a 512 MB buffer (evicts everything), then read a second 256 MB
+    buffer, so that the ~126 MB of dirty lines the write leaves behind are written back before the timed kernel
+    starts instead of competing with it for HBM."""
+
+    def __init__(self, dev):
+        import torch
+        self.w = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+        self.r = torch.zeros(L2_FLUSH_BYTES // 8, dtype=torch.int32, device=dev)
+
+    def zero_(self):
+        self.w.zero_()
+        self.r.sum()
+
+
 def _timed_reps(fn, reps, warmup, flush=None):
     """Per-rep CUDA-event times (seconds) on the current stream, optional L2 flush between reps."""
     import torch
@@ -250,7 +269,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
     peaks = _peaks()
     K, W = args.steps, max(3, args.warmup)
-    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    flush = L2Flush(dev)
 
     sampler = ClockSampler(local)
     with sampler:
@@ -302,7 +321,7 @@ def run_ours(args):
         e2e["seconds"] = max_over_ranks(e2e["seconds"], dev)
         e2e_value = job_throughput(tokens, e2e.pop("seconds"), world)
 
-        sweep, fits, roofline, extra, cpu = [], [], None, {}, None
+        sweep, fits, roofline, extra, cpu, kappa = [], [], None, {}, None, None
         if rank == 0:
             # ---------------- per-r table at the config's n_tok (cold L2 via flush), roofline fractions
             for p in preps:
@@ -322,6 +341,8 @@ def run_ours(args):
                         "roofline_time_frac": float(np.sum(attn_roof) / np.sum(attn_sec)),
                         "pure_decode_r1": {"achieved": dec["achieved_GBps"], "frac": dec["achieved_GBps"] / peaks["hbm"],
                                            "launch_us": dec["T_attn_us_median"], "note": "C2 r=1.0 alone, cold L2"}}
+            # ---------------- N1 kappa / N3 exclusive-vs-mixed (post-processing of the sweep + two extra launches per r)
+            kappa = _kappa_and_exclusive(preps, sweep, dev, W, max(3, args.reps // 2), flush)
             # ---------------- alpha/beta per r through the library's step timer (a8)
             if not args.no_fit:
                 fits = _fit_sweep(dev, W, args.reps, flush)
@@ -339,10 +360,10 @@ def run_ours(args):
                 "config": {"workload": "C2 Qwen3-4B-shaped attention layer (32/8/128, block 16), n_tok=2048/step, "
                                        "decode ctx 16, 512-token prompts, r cycled 0.0..1.0 over the K steps",
                            "n_tok": 2048, "r_grid": R_GRID, "l2": "inputs larger than L2: 11 batches x 0.5 GB pools "
-                           "cycled; per-r table uses a 512 MB L2 flush between reps", "multi_gpu": "replicas only"},
+                           "cycled; per-r table: L2 flushed between reps (512 MB write + 256 MB read)", "multi_gpu": "replicas only"},
                 "e2e": {"value": e2e_value, "unit": UNIT, **e2e},
                 "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
-                "sweep": sweep, "fits": fits, "other_configs": extra, "peaks": peaks}
+                "sweep": sweep, "fits": fits, "kappa": kappa, "other_configs": extra, "peaks": peaks}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -380,6 +401,51 @@ def _e2e(preps, K, W, dev):
     bo = np.mean([h["out"].numel() * h["out"].element_size() for h in host])
     return {"seconds": dt, "h2d_bytes_per_step": int(bi), "d2h_bytes_per_step": int(bo),
             "includes": "H2D inputs+descriptors, pa_plan, kv_append, batch_attention, D2H output; wall clock"}
+
+
+def _split_parts(batch):
+    """The decode-only and the prefill-only half of a mixed batch (same sequences, same seed) — SURVEY §8(f) N3."""
+    from paper_2606_00516_b200.synth import workloads
+    nd = batch.num_decode_seqs
+    q, c = batch.q_lens, batch.context_lens
+    dec = workloads.make_batch(batch.name + "-dec", batch.shape, batch.seed, q[:nd], c[:nd], nd,
+                               num_blocks=batch.num_blocks) if nd > 0 else None
+    pre = workloads.make_batch(batch.name + "-pre", batch.shape, batch.seed, q[nd:], c[nd:], 0,
+                               num_blocks=batch.num_blocks) if nd < batch.n_seq else None
+    return dec, pre
+
+
+def _kappa_and_exclusive(preps, sweep, dev, W, reps, flush):
+    """N1: K(r) = c0 + c1 r + c2 r^2 and kappa = 2 c2/(c0+c1+c2) of OUR attention step time at n_tok = 2048
+    (App. A.3, Eq. 9-11) through pa_timer_kappa; gap to the linear interpolation (Eq. 10).
+    N3: the same tokens as two exclusive launches (decode-only step + prefill-only step) vs the one mixed step."""
+    pa = preps[0].pa
+    pa.timer_reset()
+    for p, pt in zip(preps, sweep):
+        pa.timer_record(round(p.batch.r, 3), p.batch.n_tok, pt["T_step_us_median"] * 1e-6)
+    (c0, c1, c2), kappa, npts = pa.timer_kappa(preps[0].batch.n_tok)
+    k0, k1 = sweep[0]["T_step_us_median"], sweep[-1]["T_step_us_median"]
+    out = {"n_tok": preps[0].batch.n_tok, "c0_us": c0 * 1e6, "c1_us": c1 * 1e6, "c2_us": c2 * 1e6, "kappa": kappa,
+           "n_points": npts, "note": "attention-only K(r) of one layer on B200 (paper: whole-model kappa -11.6 on "
+           "RTX PRO 6000, -0.69 on H200, PAPER.md:L547 — context, not comparable)", "per_r": []}
+    pools = None
+    for p, pt in zip(preps, sweep):
+        b = p.batch
+        row = {"r": pt["r"], "K_mixed_us": pt["T_step_us_median"],
+               "K_linear_interp_us": (1 - b.r) * k0 + b.r * k1,
+               "gap_us": pt["T_step_us_median"] - ((1 - b.r) * k0 + b.r * k1)}
+        dec, pre = _split_parts(b)
+        t_excl = 0.0
+        for part in (dec, pre):
+            if part is None:
+                continue
+            pp = Prepared(part, dev, pools=(p.db.k_pool, p.db.v_pool))
+            t_excl += float(np.median(_timed_reps(pp.step, reps, W, flush))) * 1e6
+            del pp
+        row["K_exclusive_two_steps_us"] = t_excl
+        row["mixed_over_exclusive"] = pt["T_step_us_median"] / t_excl if t_excl > 0 else None
+        out["per_r"].append(row)
+    return out
 
 
 def _fit_sweep(dev, W, reps, flush):
@@ -496,6 +562,28 @@ def run_reference(args):
                       "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
+def run_only(args):
+    """One configuration point by itself (used for the ncu captures in profiles/): c2:<r> | c3 | c4:<r> | c5:<variant>."""
+    import torch
+    from paper_2606_00516_b200.synth import workloads
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    kind, _, arg = args.only.partition(":")
+    if kind == "c2":
+        batch = workloads.config2(float(arg or 1.0))
+    elif kind == "c3":
+        batch = workloads.config3()
+    elif kind == "c4":
+        batch = workloads.config4(float(arg or 1.0))
+    elif kind == "c5":
+        batch = workloads.config5(arg or "r1.0", num_blocks=int(150e9 // (32 * 1024)))
+    else:
+        raise SystemExit("--only takes c2:<r> | c3 | c4:<r> | c5:<variant>")
+    big = batch.algorithmic_bytes() > 4 * (126 << 20)          # inputs larger than L2: no flush needed
+    pt = _point(Prepared(batch, dev), _peaks(), args.reps, max(1, args.warmup), None if big else L2Flush(dev))
+    print(json.dumps({"only": args.only, **pt}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -505,8 +593,11 @@ def main():
     ap.add_argument("--reps", type=int, default=20, help="timed repetitions per point of the per-r tables (R19)")
     ap.add_argument("--extended", action="store_true", help="also run C4 (up to 92 GB pools) and C5 (150 GB pool)")
     ap.add_argument("--no-fit", action="store_true", help="skip the alpha/beta n_tok sweep")
+    ap.add_argument("--only", default=None, help="run one configuration point only: c2:<r> | c3 | c4:<r> | c5:<variant>")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.only:
+        run_only(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

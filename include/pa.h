@@ -140,6 +140,13 @@ int32_t pa_timer_begin(pa_ctx* ctx, void* stream);
 int32_t pa_timer_end(pa_ctx* ctx, void* stream, double r, int32_t n_tok, double* seconds_out);
 int32_t pa_timer_record(pa_ctx* ctx, double r, int32_t n_tok, double seconds); /* add an externally timed sample */
 int32_t pa_timer_fit(pa_ctx* ctx, double r, double* alpha, double* beta, double* r2, int32_t* n_points);
+/* pa_timer_kappa (App. A.3, Eq. 9-11; L550-554 App. A.4): least-squares quadratic
+ * K(r) = c0 + c1 r + c2 r^2 through the per-r MEDIAN step times recorded at this n_tok (one point per distinct r key,
+ * r = key/1000), and the interference convexity index kappa = 2 c2 / (c0 + c1 + c2).  c[3] and kappa are host
+ * outputs (seconds / dimensionless); *n_points = distinct r keys used.  PA_ERR_TIMER with < 3 distinct r, or if the
+ * normal equations are singular or c0 + c1 + c2 == 0.  The gap of Eq. 10, K(r) - [(1-r)K(0) + rK(1)], is
+ * -c2 r (1 - r).  Host arithmetic only (fp64); no device work. */
+int32_t pa_timer_kappa(pa_ctx* ctx, int32_t n_tok, double* c, double* kappa, int32_t* n_points);
 int32_t pa_timer_reset(pa_ctx* ctx);
 
 /* Introspection of the last plan (host ints; for bench.py's launch accounting and the tests).

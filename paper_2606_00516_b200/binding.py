@@ -20,7 +20,7 @@ PA_FLAG_DEBUG_SIMPLE = 1
 
 EXPORTS = ["pa_create", "pa_destroy", "pa_workspace_bytes", "pa_kv_pool_bytes", "pa_kv_append", "pa_plan",
            "pa_batch_attention", "pa_kv_gather", "pa_timer_begin", "pa_timer_end", "pa_timer_record",
-           "pa_timer_fit", "pa_timer_reset", "pa_plan_info", "pa_last_error"]
+           "pa_timer_fit", "pa_timer_kappa", "pa_timer_reset", "pa_plan_info", "pa_last_error"]
 
 
 class PaError(RuntimeError):
@@ -62,6 +62,7 @@ def load_library() -> C.CDLL:
         lib.pa_timer_end.argtypes = [vp, vp, f64, i32, C.POINTER(f64)]
         lib.pa_timer_record.argtypes = [vp, f64, i32, f64]
         lib.pa_timer_fit.argtypes = [vp, f64, C.POINTER(f64), C.POINTER(f64), C.POINTER(f64), C.POINTER(i32)]
+        lib.pa_timer_kappa.argtypes = [vp, i32, C.POINTER(f64), C.POINTER(f64), C.POINTER(i32)]
         lib.pa_timer_reset.argtypes = [vp]
         lib.pa_plan_info.argtypes = [vp, i32]
         lib.pa_plan_info.restype = i64
@@ -166,6 +167,12 @@ class PagedAttention:
         a, b, r2, n = C.c_double(), C.c_double(), C.c_double(), C.c_int32()
         self._check(self.lib.pa_timer_fit(self.ctx, r, C.byref(a), C.byref(b), C.byref(r2), C.byref(n)))
         return a.value, b.value, r2.value, n.value
+
+    def timer_kappa(self, n_tok: int):
+        """(c0, c1, c2), kappa, n_points of K(r) = c0 + c1 r + c2 r^2 at this n_tok (App. A.3, Eq. 9-11)."""
+        c, k, n = (C.c_double * 3)(), C.c_double(), C.c_int32()
+        self._check(self.lib.pa_timer_kappa(self.ctx, n_tok, c, C.byref(k), C.byref(n)))
+        return (c[0], c[1], c[2]), k.value, n.value
 
     def timer_reset(self):
         self._check(self.lib.pa_timer_reset(self.ctx))

@@ -571,6 +571,47 @@ int32_t pa_timer_fit(pa_ctx* ctx, double r, double* alpha, double* beta, double*
     return PA_OK;
 }
 
+// N1: quadratic fit of K(r) at fixed n_tok and kappa = 2 c2 / (c0 + c1 + c2)  (App. A.3, Eq. 9-11)
+int32_t pa_timer_kappa(pa_ctx* ctx, int32_t n_tok, double* c, double* kappa, int32_t* n_points) {
+    if (!ctx || !c || !kappa) return PA_ERR_INVALID;
+    std::vector<double> x, y;
+    for (auto& rk : ctx->samples) {
+        auto it = rk.second.find(n_tok);
+        if (it == rk.second.end() || it->second.empty()) continue;
+        x.push_back(rk.first / 1000.0);
+        y.push_back(median(it->second));
+    }
+    const int n = (int)x.size();
+    if (n_points) *n_points = n;
+    if (n < 3) return fail(ctx, PA_ERR_TIMER, "pa_timer_kappa: fewer than 3 distinct r at this n_tok");
+    // normal equations of the 3-parameter least squares, solved by Gaussian elimination with partial pivoting
+    double A[3][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};
+    for (int i = 0; i < n; ++i) {
+        const double p[3] = {1.0, x[i], x[i] * x[i]};
+        for (int a = 0; a < 3; ++a) {
+            for (int b = 0; b < 3; ++b) A[a][b] += p[a] * p[b];
+            A[a][3] += p[a] * y[i];
+        }
+    }
+    for (int col = 0; col < 3; ++col) {
+        int piv = col;
+        for (int r = col + 1; r < 3; ++r)
+            if (std::fabs(A[r][col]) > std::fabs(A[piv][col])) piv = r;
+        if (std::fabs(A[piv][col]) < 1e-300) return fail(ctx, PA_ERR_TIMER, "pa_timer_kappa: singular system");
+        for (int k = 0; k < 4; ++k) std::swap(A[col][k], A[piv][k]);
+        for (int r = 0; r < 3; ++r) {
+            if (r == col) continue;
+            const double f = A[r][col] / A[col][col];
+            for (int k = col; k < 4; ++k) A[r][k] -= f * A[col][k];
+        }
+    }
+    for (int a = 0; a < 3; ++a) c[a] = A[a][3] / A[a][a];
+    const double k1 = c[0] + c[1] + c[2];
+    if (k1 == 0.0) return fail(ctx, PA_ERR_TIMER, "pa_timer_kappa: K(1) == 0");
+    *kappa = 2.0 * c[2] / k1;
+    return PA_OK;
+}
+
 int32_t pa_timer_reset(pa_ctx* ctx) {
     if (!ctx) return PA_ERR_INVALID;
     ctx->samples.clear();

@@ -167,8 +167,8 @@ __device__ __forceinline__ uint64_t fsub2(uint64_t a, uint64_t b) {
 }
 // 2^x for a pair, x in [-127, 127], on the FMA pipe instead of the 16-lane MUFU: floor by a round-down magic add,
 // degree-3 minimax polynomial of 2^f on [0,1) (max relative error 8.6e-5, below the bf16 rounding of P), exponent
-// inserted with an integer add.  The prefill softmax is MUFU-bound; a share of its exponentials
-// goes through here so that the MUFU and FMA pipes split the work.
+// inserted with an integer add.  Optional path of the prefill softmax (see kPolyMask in pa_prefill.cuh: off by
+// default, because the softmax groups turned out issue-bound, not MUFU-bound, on B200).
 __device__ __forceinline__ void exp2_poly2(uint64_t x, float& p0, float& p1) {
     const uint64_t xr = fadd2_rm(x, pack_f2(12582912.f, 12582912.f));        // 1.5·2^23 + floor(x)
     const uint64_t fl = fadd2(xr, pack_f2(-12582912.f, -12582912.f));         // floor(x), exact

@@ -240,3 +240,24 @@ def test_timer_fit_matches_oracle_fit():
     pa.timer_begin()
     sec = pa.timer_end(0.7, 128)
     assert 0 <= sec < 1.0
+
+
+def test_timer_kappa_matches_oracle_quadratic():
+    """N1 (App. A.3, Eq. 9-11): the library's quadratic fit of K(r) and kappa vs the oracle's."""
+    pa = binding.PagedAttention(8, 2, 128, 64, 4, 64, 8)
+    rng = np.random.default_rng(5)
+    rs = [i / 10 for i in range(11)]
+    Ks = []
+    for r in rs:
+        reps = 20e-6 + 30e-6 * r - 12e-6 * r * r + rng.normal(0, 2e-7, 9)
+        for t in reps:
+            pa.timer_record(r, 2048, float(t))
+        pa.timer_record(r, 512, 1e-6)                      # other n_tok: must not enter the fit
+        Ks.append(float(np.median(reps)))
+    c, kappa, npts = pa.timer_kappa(2048)
+    oc, okappa = oracle.quadratic_kappa(np.array(rs), np.array(Ks))
+    assert npts == 11
+    assert np.allclose(c, oc, rtol=1e-9, atol=1e-15) and abs(kappa - okappa) < 1e-9
+    with pytest.raises(binding.PaError) as e:
+        pa.timer_kappa(4096)                               # no samples at this n_tok
+    assert e.value.code == binding.PA_ERR_TIMER
