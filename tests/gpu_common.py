@@ -81,3 +81,58 @@ def check_close(out_bits: np.ndarray, ref: np.ndarray, what=""):
     assert err.max() <= MAX_ABS, f"{what}: max abs err {err.max():.4g} > {MAX_ABS} at {np.unravel_index(err.argmax(), err.shape)}"
     assert err.mean() <= MEAN_ABS, f"{what}: mean abs err {err.mean():.4g} > {MEAN_ABS}"
     return float(err.max()), float(err.mean())
+
+
+def check_sampled_sequences(batch, d, seqs, prefill_row_stride=16, n_threads=8, what=""):
+    """Full-size parity on a sample of sequences without a host copy of the pool: the sampled sequences' blocks
+    are gathered from the DEVICE pool (post-append) into a compact host pool with relabelled block ids, and the
+    oracle runs on the mini-batch made of those sequences only.  Legitimate by the oracle's own invariances
+    (P9 block relabelling, P11 batch permutation/subsetting).  Also checks kv_append placement bit-exactly for the
+    sampled sequences.  Prefill chunks are checked on every `prefill_row_stride`-th row plus first and last."""
+    sh = batch.shape
+    b = sh.block_size
+    seqs = [int(s) for s in seqs]
+    dec = [s for s in seqs if s < batch.num_decode_seqs]
+    pre = [s for s in seqs if s >= batch.num_decode_seqs]
+    order = dec + pre                                            # decode first (R11)
+    q_lens = batch.q_lens[order]
+    ctx = batch.context_lens[order]
+    kv = ctx.astype(np.int64) + q_lens
+    nblk = (kv + b - 1) // b
+    width = int(nblk.max())
+    tables = np.full((len(order), width), -1, dtype=np.int32)
+    phys = []
+    off = 0
+    for i, s in enumerate(order):
+        n = int(nblk[i])
+        tables[i, :n] = np.arange(off, off + n, dtype=np.int32)
+        phys.append(batch.block_tables[s, :n].astype(np.int64))
+        off += n
+    phys = torch.from_numpy(np.concatenate(phys)).to(d["k_pool"].device)
+    kp = sdev.bits(d["k_pool"].index_select(0, phys))            # [off, Hkv, b, D] compact, post-append
+    vp = sdev.bits(d["v_pool"].index_select(0, phys))
+    rows_src = np.concatenate([np.arange(batch.cu_seqlens_q[s], batch.cu_seqlens_q[s + 1]) for s in order])
+    idx = torch.from_numpy(rows_src).to(d["q"].device)
+    q = sdev.bits(d["q"].index_select(0, idx))
+    out = sdev.bits(d["out"].index_select(0, idx))
+    k_new = sdev.bits(d["k_new"].index_select(0, idx))
+    v_new = sdev.bits(d["v_new"].index_select(0, idx))
+    cu = np.zeros(len(order) + 1, dtype=np.int32)
+    np.cumsum(q_lens, out=cu[1:])
+    # ---- append placement, bit-exact: token j of sequence i sits in slot(ctx_i + j)
+    for i in range(len(order)):
+        t = ctx[i] + np.arange(q_lens[i])
+        blk = tables[i, t // b]
+        assert (kp[blk, :, t % b, :] == k_new[cu[i]:cu[i + 1]]).all(), f"{what}: K append placement, seq {order[i]}"
+        assert (vp[blk, :, t % b, :] == v_new[cu[i]:cu[i + 1]]).all(), f"{what}: V append placement, seq {order[i]}"
+    # ---- attention on the sampled rows
+    rows = []
+    for i in range(len(order)):
+        r = np.arange(cu[i], cu[i + 1])
+        if i >= len(dec) and len(r) > 2:
+            r = np.unique(np.concatenate([r[::prefill_row_stride], r[:1], r[-1:]]))
+        rows.append(r)
+    rows = np.concatenate(rows).astype(np.int64)
+    ref = oracle.attention(oracle_shape(batch), q, kp, vp, cu, ctx, tables, batch.softmax_scale, rows=rows,
+                           n_threads=n_threads)
+    return check_close(out[rows], ref, what)

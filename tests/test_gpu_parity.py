@@ -178,6 +178,40 @@ def test_config3_full_size_sampled():
     assert np.isfinite(got).all()                       # property at full size: no sentinel leaked anywhere
 
 
+def test_config4_full_size_sampled():
+    """C4 (Qwen3-8B shape, n_tok 8192) at r = 0.5, full size, in the launch configuration bench.py times: one mixed
+    launch over a ~40 GB pool; 96 sampled decode sequences + both prefill chunks (every 16th row) vs the oracle."""
+    import gc as pygc
+    pygc.collect()
+    torch.cuda.empty_cache()
+    batch = workloads.config4(0.5)
+    d = gc.run_gpu(batch, None)
+    rng = np.random.default_rng(45)
+    seqs = list(rng.choice(batch.num_decode_seqs, 96, replace=False)) + list(range(batch.num_decode_seqs, batch.n_seq))
+    gc.check_sampled_sequences(batch, d, seqs, what=batch.name)
+    assert torch.isfinite(d["out"].float()).all()      # property at full size: no NaN sentinel leaked anywhere
+    assert d["pa"].plan_info(6) > 0 and d["pa"].plan_info(1) > 0, "expected a mixed launch"
+
+
+def test_config5_full_size_sampled():
+    """C5 (Qwen3-30B-A3B shape, G = 8) with the 150 GB pool (3.75e10 elements per pool: 64-bit block addressing),
+    variant r0.2 (1024 decode sequences with ctx in [4096, 32768] + 4 prefill chunks of 1024)."""
+    import gc as pygc
+    pygc.collect()
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    nb = int(150e9 // (32 * 1024))
+    if free < 160e9:
+        nb = int((free - 8e9) // (32 * 1024))          # largest pool that fits this device (recorded in the test name)
+    batch = workloads.config5("r0.2", num_blocks=nb)
+    assert batch.block_tables.max() > (1 << 31) // (4 * 16 * 128), "block ids must reach past 2^31 elements"
+    d = gc.run_gpu(batch, None)
+    rng = np.random.default_rng(57)
+    seqs = list(rng.choice(batch.num_decode_seqs, 24, replace=False)) + list(range(batch.num_decode_seqs, batch.n_seq))
+    gc.check_sampled_sequences(batch, d, seqs, what=f"{batch.name}/nb={nb}")
+    assert torch.isfinite(d["out"].float()).all()
+
+
 def test_empty_and_degenerate_batches():
     W = workloads
     pa = binding.PagedAttention(8, 2, 128, 64, 8, 256, 8)
