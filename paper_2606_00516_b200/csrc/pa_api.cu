@@ -313,11 +313,13 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     const int n_dec = simple_all ? 0 : num_decode_seqs;
     int64_t total_blocks = 0;
     for (int s = 0; s < n_dec; ++s) total_blocks += ((int64_t)h_ctx[s] + 1 + kBlock - 1) / kBlock * Hkv;
-    // ---- CTA partition of the single launch (a7): share the SMs in proportion to the estimated CTA-time of the
-    // two roles.  Prefill: per unit a fill of ~1.5 us plus ~1.4 us per (q-head tile, KV tile) pair (measured
-    // softmax/MMA pipeline rate).  Decode: the larger of its HBM time on all SMs and the per-stream latency time
-    // (~3 us per item + bytes at ~16 GB/s per stream, 8 streams per CTA).  CTAs switch role when their own queue
-    // runs dry, so the split only has to be roughly right (measured flat within +-30 % of this choice).
+    // ---- CTA partition of the single launch (a7): share the SMs in proportion to the CTA-time of the two roles,
+    // from rates measured with per-CTA timestamps on B200.  Prefill: ~7 us per unit (hand-out, Q/K fill, two-pass
+    // first tile, epilogue) + ~0.95 us per (q-head tile, KV tile) pair.  Decode: ~2 us per item and stream plus its
+    // bytes at ~16 GB/s per stream (8 streams per CTA) when latency-bound; when its HBM time on all SMs is the
+    // larger figure decode is bandwidth-bound and ~96 CTAs saturate HBM, so prefill may take as many CTAs as it
+    // needs to finish within the decode's HBM time.  CTAs switch role when their own queue runs dry, so the split
+    // only has to be roughly right.
     const int sms = ctx->num_sms;
     int32_t pre_ctas = 0;
     if (n_units > 0 && total_blocks > 0) {
@@ -325,12 +327,19 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
         double t_pre = 0.0;   // CTA-microseconds
         for (const PreTile& t : tile_vec) {
             const double n_kv = std::ceil((double)(t.ctx + t.q_begin + t.q_rows) / KT);
-            t_pre += (double)Hkv * (head_groups * 1.5 + n_kv * G * 1.4);
+            t_pre += (double)Hkv * (head_groups * 7.0 + n_kv * G * 0.95);
         }
         const double dec_bytes = (double)total_blocks * kBlock * D * 2 * 2;
         const double n_groups = (double)n_dec * Hkv;
-        const double t_dec = std::max(sms * dec_bytes / 6.5e12 * 1e6, n_groups * 3.0 / kDecodeWarps + dec_bytes / 16e9 / kDecodeWarps * 1e6);
-        pre_ctas = (int32_t)std::lround(sms * t_pre / (t_pre + t_dec));
+        const double t_hbm = dec_bytes / 6.5e12 * 1e6;                                        // us, all SMs
+        const double t_lat = n_groups * 2.0 / kDecodeWarps + dec_bytes / 16e9 / kDecodeWarps * 1e6;   // CTA-us
+        if (sms * t_hbm >= t_lat) {
+            const double need = t_pre / t_hbm;                                               // CTAs to hide prefill under decode
+            pre_ctas = (int32_t)std::lround(std::min<double>(need, sms - 96));
+            pre_ctas = std::max(pre_ctas, (int32_t)std::lround(sms * t_pre / (t_pre + sms * t_hbm)));
+        } else {
+            pre_ctas = (int32_t)std::lround(sms * t_pre / (t_pre + t_lat));
+        }
         pre_ctas = env_int("PA_PREFILL_CTAS", pre_ctas);
         pre_ctas = std::max(1, std::min({pre_ctas, sms - 1, n_units}));
     } else if (n_units > 0) {

@@ -58,14 +58,12 @@ struct DecodeCfg {
 constexpr int kDecodeProducerWarps = 4;                              // warps 0-3
 constexpr int kStreamsPerProducer = kDecodeWarps / kDecodeProducerWarps;
 
-// one thread, once per CTA, before the roles start
+// one thread per stream, once per CTA, before the roles start
 template <int D>
-__device__ __forceinline__ void decode_init_barriers(uint8_t* dec_aux) {
+__device__ __forceinline__ void decode_init_barriers(uint8_t* dec_aux, int s) {
     using Cfg = DecodeCfg<D>;
-    for (int s = 0; s < kDecodeWarps; ++s) {
-        const uint32_t a = smem_u32(dec_aux + s * Cfg::kAuxBytes);
-        for (int i = 0; i < 2 * Cfg::kRing + 2 * Cfg::kFifo; ++i) mbar_init(a + 8 * i, 1);
-    }
+    const uint32_t a = smem_u32(dec_aux + s * Cfg::kAuxBytes);
+    for (int i = 0; i < 2 * Cfg::kRing + 2 * Cfg::kFifo; ++i) mbar_init(a + 8 * i, 1);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -436,6 +434,10 @@ __device__ __forceinline__ void decode_role(const AttnParams& p, const CUtensorM
         const int s = warp - kDecodeProducerWarps;
         decode_consumer<D>(p, tiles + s * Cfg::kStreamBytes, dec_aux + s * Cfg::kAuxBytes);
     }
+    // The producer warps ran with two lanes in their own control flow: reconverge every warp before the caller's
+    // __syncthreads().  A warp that reaches a CTA barrier in two pieces is counted twice, and the barrier would
+    // release while consumer warps are still reading the ring (measured: thread 0 passed it ~7 us early).
+    __syncwarp();
 }
 
 }  // namespace pa

@@ -83,6 +83,8 @@ __global__ void __launch_bounds__(256) pa_kv_gather_kernel(const int4* __restric
 cudaError_t launch_kv_append(const LaunchShape& sh, const void* k_new, const void* v_new, void* k_pool, void* v_pool,
                              const int32_t* cu, const int32_t* ctx, const int32_t* bt, int32_t n_seq, int32_t n_tok,
                              cudaStream_t stream) {
+    // launched normally: measured on B200, launching kv_append itself with programmatic stream serialization (its
+    // CTAs queued under the previous attention launch) made the step 4 us SLOWER
     const int warps = 8;
     dim3 grid((n_tok + warps - 1) / warps), block(warps * 32);
     if (sh.D == 128)
@@ -135,17 +137,22 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
     PrefillCtrl* ctrl = reinterpret_cast<PrefillCtrl*>(tiles + kTileRegion);
     uint8_t* dec_aux = tiles + kTileRegion + kCtrlBytes;
     const PlanView& pl = p.plan;
-    if (threadIdx.x == 0) {
+    // set-up spread over threads (it is on the critical path of microsecond-scale launches): thread 0 the prefill
+    // barriers, threads 32.. one decode stream each, thread 64 the descriptor prefetches
+    if (threadIdx.x == 0 && pl.n_units > 0) prefill_init_barriers(ctrl);
+    if (threadIdx.x >= 32 && threadIdx.x < 32 + kDecodeWarps && pl.n_bundles > 0)
+        decode_init_barriers<D>(dec_aux, (int)threadIdx.x - 32);
+    if (threadIdx.x == 64) {
         tma_prefetch_desc(&tmK);
         tma_prefetch_desc(&tmV);
-        if (pl.n_units > 0) {
-            tma_prefetch_desc(&tmQ);
-            prefill_init_barriers(ctrl);
-        }
+        if (pl.n_units > 0) tma_prefetch_desc(&tmQ);
         if (pl.n_bundles > 0) {
             tma_prefetch_desc(&tmQd);
-            decode_init_barriers<D>(dec_aux);
+            tma_prefetch_desc(&tails.k[0]);
+            tma_prefetch_desc(&tails.v[0]);
         }
+    }
+    if (threadIdx.x < 64) {
         fence_mbar_init();
         fence_proxy_async();
     }
