@@ -321,7 +321,7 @@ def run_ours(args):
         e2e["seconds"] = max_over_ranks(e2e["seconds"], dev)
         e2e_value = job_throughput(tokens, e2e.pop("seconds"), world)
 
-        sweep, fits, roofline, extra, cpu, kappa = [], [], None, {}, None, None
+        sweep, fits, roofline, extra, cpu, kappa, ctx_sweep = [], [], None, {}, None, None, None
         if rank == 0:
             # ---------------- per-r table at the config's n_tok (cold L2 via flush), roofline fractions
             for p in preps:
@@ -346,6 +346,7 @@ def run_ours(args):
             # ---------------- alpha/beta per r through the library's step timer (a8)
             if not args.no_fit:
                 fits = _fit_sweep(dev, W, args.reps, flush)
+                ctx_sweep = _ctx_sweep(dev, peaks, W, max(3, args.reps // 2), flush)
             # ---------------- bandwidth-bound decode (C3) and, with --extended, C4 / C5
             del preps
             torch.cuda.empty_cache()
@@ -363,7 +364,7 @@ def run_ours(args):
                            "cycled; per-r table: L2 flushed between reps (512 MB write + 256 MB read)", "multi_gpu": "replicas only"},
                 "e2e": {"value": e2e_value, "unit": UNIT, **e2e},
                 "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
-                "sweep": sweep, "fits": fits, "kappa": kappa, "other_configs": extra, "peaks": peaks}
+                "sweep": sweep, "fits": fits, "kappa": kappa, "ctx_sweep": ctx_sweep, "other_configs": extra, "peaks": peaks}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -380,15 +381,36 @@ def _e2e(preps, K, W, dev):
         h["out"] = torch.empty_like(d.out, device="cpu").pin_memory()
         host.append(h)
 
-    def one(i):
-        p, h = preps[i % len(preps)], host[i % len(preps)]
-        d, b = p.db, p.batch
-        for k in ("q", "k_new", "v_new", "cu_seqlens_q", "context_lens", "block_tables"):
-            getattr(d, k).copy_(h[k], non_blocking=True)
-        p.pa.plan(b.cu_seqlens_q, b.context_lens, b.n_seq, b.num_decode_seqs)
-        p.step()
-        h["out"].copy_(d.out, non_blocking=True)
+    # Three streams, as a serving engine would run it: the H2D of step i+1 and the D2H of step i-1 overlap the
+    # kernels of step i (every r-batch has its own device buffers, so the only hazards are a batch's own previous use).
+    n = len(preps)
+    s_in, s_run, s_out = torch.cuda.Stream(dev), torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+    last_out = [None] * n          # event: the previous D2H of this batch's output buffer has finished
 
+    def one(i):
+        p, h = preps[i % n], host[i % n]
+        d, b = p.db, p.batch
+        with torch.cuda.stream(s_in):
+            if last_out[i % n] is not None:
+                s_in.wait_event(last_out[i % n])        # inputs of this batch are being overwritten: its last step is done
+            for k in ("q", "k_new", "v_new", "cu_seqlens_q", "context_lens", "block_tables"):
+                getattr(d, k).copy_(h[k], non_blocking=True)
+            e_in = torch.cuda.Event()
+            e_in.record(s_in)
+        with torch.cuda.stream(s_run):
+            s_run.wait_event(e_in)
+            p.pa.plan(b.cu_seqlens_q, b.context_lens, b.n_seq, b.num_decode_seqs)
+            p.step()
+            e_run = torch.cuda.Event()
+            e_run.record(s_run)
+        with torch.cuda.stream(s_out):
+            s_out.wait_event(e_run)
+            h["out"].copy_(d.out, non_blocking=True)
+            e_out = torch.cuda.Event()
+            e_out.record(s_out)
+        last_out[i % n] = e_out
+
+    torch.cuda.synchronize()
     for i in range(W):
         one(i)
     torch.cuda.synchronize()
@@ -400,7 +422,8 @@ def _e2e(preps, K, W, dev):
     bi = np.mean([sum(h[k].numel() * h[k].element_size() for k in h if k != "out") for h in host])
     bo = np.mean([h["out"].numel() * h["out"].element_size() for h in host])
     return {"seconds": dt, "h2d_bytes_per_step": int(bi), "d2h_bytes_per_step": int(bo),
-            "includes": "H2D inputs+descriptors, pa_plan, kv_append, batch_attention, D2H output; wall clock"}
+            "includes": "per step: H2D inputs+descriptors (pinned), pa_plan, kv_append, batch_attention, D2H output; copies on "
+                        "their own streams overlap the neighbouring steps' kernels; wall clock over the K steps"}
 
 
 def _split_parts(batch):
@@ -445,6 +468,28 @@ def _kappa_and_exclusive(preps, sweep, dev, W, reps, flush):
         row["K_exclusive_two_steps_us"] = t_excl
         row["mixed_over_exclusive"] = pt["T_step_us_median"] / t_excl if t_excl > 0 else None
         out["per_r"].append(row)
+    return out
+
+
+def _ctx_sweep(dev, peaks, W, reps, flush):
+    """N2 (Fig. 10 analogue): n_tok = 1024, decode ctx in {16, 64, 128, 256, 512},
+    r = 0 ... 1.  The paper's observations to check: time grows monotonically with ctx at fixed r > 0, and the ctx
+    curves meet at r = 0 ("no KV cache is accessed")."""
+    from paper_2606_00516_b200.synth import workloads
+    out = {"n_tok": 1024, "ctx": [16, 64, 128, 256, 512], "r": [0.0, 0.2, 0.4, 0.6, 0.8, 1.0], "T_step_us": {}}
+    pools = None
+    for ctx in out["ctx"]:
+        row = []
+        for r in out["r"]:
+            b = workloads.config2(r, n_tok=1024, ctx=ctx, num_blocks=40960)
+            p = Prepared(b, dev, pools=pools)
+            pools = (p.db.k_pool, p.db.v_pool)
+            row.append(float(np.median(_timed_reps(p.step, reps, W, flush))) * 1e6)
+            del p
+        out["T_step_us"][str(ctx)] = row
+    cols = np.array([out["T_step_us"][str(c)] for c in out["ctx"]])
+    out["monotone_in_ctx_for_r_ge_0.4"] = bool((np.diff(cols[:, 2:], axis=0) > -1.0).all())   # 1 us timing slack
+    out["spread_at_r0_us"] = float(cols[:, 0].max() - cols[:, 0].min())
     return out
 
 

@@ -175,9 +175,11 @@ int32_t pa_create(pa_ctx** out, const pa_config* cfg) {
     }
     // ---- workspace layout
     ctx->max_workers = ctx->num_sms * kDecodeWarps;
-    ctx->max_bundles = ctx->max_workers * 5 + 8;   // k <= 4 bundles per worker; unsplit short groups close bundles up to 1/8 early
+    // k <= 4 equal bundles per worker, plus the bundles that uncut short groups close early (at most one per group)
+    const int32_t eq_bundles = ctx->max_workers * 5 + 8;
+    ctx->max_bundles = eq_bundles + cfg->max_seqs * cfg->num_kv_heads;
     ctx->max_items = cfg->max_seqs * cfg->num_kv_heads + ctx->max_bundles + 8;
-    ctx->max_split = 2 * ctx->max_bundles;
+    ctx->max_split = 2 * eq_bundles;          // only groups cut by a bundle boundary have partials
     ctx->max_tiles = cfg->max_tokens / kQTile + cfg->max_seqs + 1;
     int64_t off = 0;
     ctx->off_counters = off;
@@ -369,10 +371,10 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
             const int32_t nblk = (kv_len + kBlock - 1) / kBlock;
             for (int g = 0; g < Hkv; ++g) {
                 int32_t pos = 0, first_item = n_items;
-                if ((nblk <= 2 || (int64_t)nblk * 4 <= target) && cur + nblk > target) {
-                    // a short group is never cut (partials + merge would cost more than the imbalance, which is
-                    // bounded by a quarter bundle): it goes whole into this bundle or the next, whichever ends
-                    // nearer the target
+                if ((nblk <= 16 || (int64_t)nblk * 4 <= target) && cur + nblk > target) {
+                    // a short group (<= 256 keys, or a quarter bundle) is never cut: partials + merge would cost
+                    // more than the imbalance it leaves (a microsecond or two of streaming); it goes whole into this
+                    // bundle or the next, whichever ends nearer the target
                     if (cur + nblk - target > target - cur) {
                         bundle_start.push_back(n_items);
                         cur = 0;

@@ -165,6 +165,18 @@ def test_config2_parity(r):
     gc.check_close(sdev.bits(d["out"])[rows], ref, batch.name)
 
 
+@pytest.mark.parametrize("ctx,r", [(128, 0.8), (64, 0.6), (256, 0.2), (512, 1.0)])
+def test_ctx_sweep_points_parity(ctx, r):
+    """N2 shapes (n_tok 1024, decode ctx 64..512): mixed launches whose decode groups are short enough never to be
+    cut, so bundles close per group (the bundle list must hold one bundle per group) — sampled rows vs the oracle."""
+    batch = workloads.config2(r, n_tok=1024, ctx=ctx, num_blocks=40960)
+    d = gc.run_gpu(batch, None)
+    rng = np.random.default_rng(ctx)
+    seqs = list(rng.choice(batch.num_decode_seqs, 48, replace=False)) + list(range(batch.num_decode_seqs, batch.n_seq))
+    gc.check_sampled_sequences(batch, d, seqs, prefill_row_stride=8, what=batch.name + f"/ctx{ctx}")
+    assert torch.isfinite(d["out"].float()).all()
+
+
 def test_config3_full_size_sampled():
     batch = workloads.config3()
     d = gc.run_gpu(batch, None)
