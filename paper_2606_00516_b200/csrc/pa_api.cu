@@ -353,13 +353,13 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     std::vector<int32_t> bundle_start;
     if (total_blocks > 0) {
         // workers that start in the decode role; in a mixed launch the prefill CTAs join through the queue when
-        // their units run out, so bundles are made finer (>= 4 per worker) and the tail balances dynamically
+        // their units run out, so bundles are made finer (>= 2 per worker) and the tail balances dynamically
         const int64_t W = (int64_t)(sms - pre_ctas) * kDecodeWarps;
         const bool mixed = pre_ctas > 0;
         const double kv_bytes = (double)total_blocks * kBlock * D * 2 * 2;
         const double part_bytes = (double)G * D * 4 * 2;
         int k = (int)std::floor(0.01 * kv_bytes / ((double)W * part_bytes));
-        k = std::max(mixed ? 4 : 1, std::min(4, k));
+        k = std::max(mixed ? 2 : 1, std::min(4, k));      // measured on C2: 2 per worker beats 1, 3 and 4 in mixed launches
         k = std::max(1, std::min(4, env_int("PA_BUNDLE_K", k)));
         const int64_t min_blocks = std::max(1, env_int("PA_MIN_BUNDLE_BLOCKS", 2));
         const int64_t target = std::max(min_blocks, (total_blocks + W * k - 1) / (W * k));
