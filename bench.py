@@ -17,7 +17,7 @@ and the descriptors, pa_plan, kv_append, batch_attention, D2H of the output, per
 Also reported: per-r table (tokens/s, achieved GB/s, roofline fraction, alpha/beta/R² of
 T = alpha + beta·n_tok fitted through pa_timer_*), kappa and the mixed-vs-exclusive comparison
 (SURVEY §8(f) N1/N3), the bandwidth-bound C3 (Gemma-3-1B decode) line, with --extended C4 (Qwen3-8B
-mixed, n_tok 8192) and C5 (Qwen3-30B-A3B, 150 GB pool); the oracle timed on the host cores
+mixed, n_tok 8192), N4 batches shaped by the paper's Table 9 length statistics and C5 (Qwen3-30B-A3B, 150 GB pool); the oracle timed on the host cores
 (cpu_baseline).  Multi-GPU: the path has no exchange step ("replicas only"): each rank
 runs the same workload on its GPU, value = Σ tokens / max-over-ranks time.
 """
@@ -564,6 +564,9 @@ def _extra_configs(dev, peaks, args, W, flush):
     if args.extended:
         for r in (0.0, 0.1, 0.5, 1.0):
             run(f"C4_qwen3_8b_r{r:.1f}", workloads.config4(r), 5, use_flush=False)
+        for name in workloads.TABLE9:                       # N4: Table 9 length statistics
+            for r in (0.5, 0.9):
+                run(f"N4_{name}_r{r:.1f}", workloads.table9_batch(name, r), 5, use_flush=False)
         pool_blocks = int(150e9 // (32 * 1024))
         for v in ("r1.0", "r0.2", "r0.059"):
             run(f"C5_qwen3_30b_a3b_{v}", workloads.config5(v, num_blocks=pool_blocks), 3, use_flush=False)

@@ -229,3 +229,47 @@ def random_batch(seed: int, shape: Shape, n_decode: int, n_prefill: int, max_ctx
     q = [1] * n_decode + list(pq)
     c = list(dc) + list(pc)
     return make_batch(f"rand-{seed}", shape, seed, q, c, n_decode, num_blocks=num_blocks)
+
+
+# ------------------------------------------------------------------------------------------------ N4
+# Length statistics of the paper's workloads (App. E.1, Table 9): input range and mean, output
+# range, mean and standard deviation.  Only these statistics are used — no dataset item is present or needed.
+# (WildChat's input columns in Table 9 count conversation turns, not tokens, so it is left out.)
+TABLE9 = {
+    "sharegpt-like": dict(in_range=(1, 20448), in_mean=105, out_range=(2, 500), out_mean=280, out_std=153),
+    "longbench-like": dict(in_range=(1000, 4000), in_mean=2492, out_range=(1, 19), out_mean=11, out_std=4),
+    "numinamath-like": dict(in_range=(16, 1395), in_mean=122, out_range=(800, 3149), out_mean=1039, out_std=228),
+}
+
+
+def _draw_lengths(rng, n: int, lo: int, hi: int, mean: float) -> np.ndarray:
+    """n integer lengths in [lo, hi] whose mean is ~`mean`: lognormal (sigma 1) shifted to `lo`, clipped at `hi`;
+    for a narrow range (mean near the middle) this is close to uniform, for a long-tailed one it is heavy-tailed."""
+    if mean - lo <= 0:
+        return np.full(n, lo, dtype=np.int64)
+    if (hi - lo) < 4 * (mean - lo):           # mean is not far below the top: uniform around it
+        half = min(mean - lo, hi - mean)
+        return rng.integers(int(mean - half), int(mean + half) + 1, n)
+    mu = math.log(mean - lo) - 0.5           # E[lognormal(mu, 1)] = exp(mu + 1/2)
+    return np.clip(lo + np.exp(rng.normal(mu, 1.0, n)), lo, hi).astype(np.int64)
+
+
+def table9_batch(name: str, r: float, n_tok: int = 2048, shape: Shape = QWEN3_8B, seed: int = 900) -> Batch:
+    """One steady-state serving step shaped like a Table 9 workload: n_dec = round(r n_tok) decode
+    sequences whose context = prompt length + tokens generated so far (uniform in [0, O)), and prefill prompts drawn
+    from the input-length statistics until the remaining token budget is filled (the last one is cut, i.e. chunked
+    prefill, PAPER.md:L437)."""
+    st = TABLE9[name]
+    rng = np.random.default_rng(seed + sorted(TABLE9).index(name) * 16 + int(round(10 * r)))
+    nd = n_decode_for(r, n_tok)
+    L = _draw_lengths(rng, nd, *st["in_range"], st["in_mean"])
+    O = np.clip(rng.normal(st["out_mean"], st["out_std"], nd), *st["out_range"]).astype(np.int64)
+    dc = L + (rng.random(nd) * O).astype(np.int64)
+    q, c = [1] * nd, list(dc)
+    left = n_tok - nd
+    while left > 0:
+        p = int(min(left, _draw_lengths(rng, 1, *st["in_range"], st["in_mean"])[0]))
+        q.append(p)
+        c.append(0)
+        left -= p
+    return make_batch(f"N4-{name}-r{r:.1f}", shape, seed, q, c, nd)

@@ -177,6 +177,21 @@ def test_ctx_sweep_points_parity(ctx, r):
     assert torch.isfinite(d["out"].float()).all()
 
 
+@pytest.mark.parametrize("name,r", [("sharegpt-like", 0.5), ("numinamath-like", 0.9), ("longbench-like", 0.5)])
+def test_table9_shaped_batches_parity(name, r):
+    """N4: steady-state steps whose context / prompt lengths follow the statistics of the paper's Table 9
+     — ragged decode contexts plus chunked prompts in one mixed launch, sampled vs the oracle."""
+    import gc as pygc
+    pygc.collect()
+    torch.cuda.empty_cache()
+    batch = workloads.table9_batch(name, r)
+    d = gc.run_gpu(batch, None)
+    rng = np.random.default_rng(9)
+    seqs = list(rng.choice(batch.num_decode_seqs, 40, replace=False)) + list(range(batch.num_decode_seqs, batch.n_seq))
+    gc.check_sampled_sequences(batch, d, seqs, prefill_row_stride=16, what=batch.name)
+    assert torch.isfinite(d["out"].float()).all()
+
+
 def test_config3_full_size_sampled():
     batch = workloads.config3()
     d = gc.run_gpu(batch, None)
