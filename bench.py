@@ -43,7 +43,7 @@ FIT_NTOK = [512, 1024, 2048, 4096]          # DESIGN R18
 L2_FLUSH_BYTES = 512 << 20
 # dram__bytes_read.sum + dram__bytes_write.sum per pa_attention_kernel launch, mean over the 11 r-batches of C2,
 # from the ncu --set full capture summarised in profiles/ (None until that capture exists)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 96044474.2
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 96011101.1
 NCU_TRAFFIC_SOURCE = "profiles/r1g_c2_cycle.md (ncu --set full, 11 launches of one r-cycle)"
 
 
