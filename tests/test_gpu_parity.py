@@ -33,6 +33,14 @@ def _small_case(name):
         return W.random_batch(204, W.GEMMA3_1B, n_decode=13, n_prefill=3, max_ctx=900, max_q=140)
     if name == "ragged-g1-d128":
         return W.random_batch(205, W.Shape(4, 4, 128), n_decode=7, n_prefill=2, max_ctx=200, max_q=70)
+    if name == "ragged-g8-d256":    # widest group at the larger head size
+        return W.random_batch(212, W.Shape(16, 2, 256), n_decode=9, n_prefill=2, max_ctx=600, max_q=200)
+    if name == "ragged-g3-d128":    # odd group: the second head group of a prefill unit has one active q-head tile
+        return W.random_batch(213, W.Shape(6, 2, 128), n_decode=10, n_prefill=3, max_ctx=500, max_q=260)
+    if name == "ragged-g5-d128":
+        return W.random_batch(214, W.Shape(5, 1, 128), n_decode=8, n_prefill=2, max_ctx=400, max_q=150)
+    if name == "ragged-g2-d256":
+        return W.random_batch(215, W.Shape(4, 2, 256), n_decode=8, n_prefill=3, max_ctx=700, max_q=300)
     if name == "edge-lens":     # kv_len in {1, 15, 16, 17, 33, 128, 129}
         return W.make_batch("edge", W.TINY, 206, [1, 1, 1, 1, 1, 1, 1, 17, 1, 128, 129],
                             [0, 14, 15, 16, 32, 127, 128, 16, 0, 0, 127], 7)
@@ -43,7 +51,8 @@ def _small_case(name):
     raise KeyError(name)
 
 
-SMALL = ["C1", "ragged-tiny", "ragged-g4-d128", "ragged-g8-d128", "ragged-g4-d256", "ragged-g1-d128", "edge-lens",
+SMALL = ["C1", "ragged-tiny", "ragged-g4-d128", "ragged-g8-d128", "ragged-g4-d256", "ragged-g1-d128", "ragged-g8-d256",
+         "ragged-g3-d128", "ragged-g5-d128", "ragged-g2-d256", "edge-lens",
          "decode-only", "prefill-only"]
 
 
@@ -135,6 +144,17 @@ def test_prefill_running_max_growth(shape_name, mode, monkeypatch):
     d = gc.run_gpu(batch, inp)
     ref, _, _ = gc.run_oracle(batch, inp)
     gc.check_close(sdev.bits(d["out"]), ref, f"growth/{shape_name}/mode{mode}")
+
+
+@pytest.mark.parametrize("shape_name,ctx", [("GEMMA3_1B", 150000), ("QWEN3_30B_A3B", 60000)])
+def test_one_long_sequence_split_over_every_worker(shape_name, ctx):
+    """A single decode sequence with a very long context: its (sequence, KV head) groups are cut into as many parts
+    as there are decode streams (hundreds per group), all merged in the launch by whichever stream arrives last."""
+    W = workloads
+    batch = W.make_batch("long1", getattr(W, shape_name), 216, [1], [ctx], 1)
+    d = gc.run_gpu(batch, None, repeat=2)
+    assert d["pa"].plan_info(2) >= 148, "expected the groups to be split across the streams"
+    gc.check_sampled_sequences(batch, d, [0], what=f"long1/{shape_name}")
 
 
 def test_repeated_launches_are_deterministic_and_reset_state():
