@@ -564,6 +564,9 @@ def _extra_configs(dev, peaks, args, W, flush):
     if args.extended:
         for r in (0.0, 0.1, 0.5, 1.0):
             run(f"C4_qwen3_8b_r{r:.1f}", workloads.config4(r), 5, use_flush=False)
+        # small batch, very long contexts: every (sequence, KV head) group is split over ~all decode streams
+        run("long_context_4x131072", workloads.make_batch("long-4x131072", workloads.QWEN3_8B, 5, [1] * 4, [131072] * 4, 4),
+            5, use_flush=False)
         for name in workloads.TABLE9:                       # N4: Table 9 length statistics
             for r in (0.5, 0.9):
                 run(f"N4_{name}_r{r:.1f}", workloads.table9_batch(name, r), 5, use_flush=False)

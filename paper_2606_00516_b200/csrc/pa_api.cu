@@ -356,10 +356,12 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
         // their units run out, so bundles are made finer (>= 2 per worker) and the tail balances dynamically
         const int64_t W = (int64_t)(sms - pre_ctas) * kDecodeWarps;
         const bool mixed = pre_ctas > 0;
+        // Bundles per worker (measured on B200): pure decode — one static bundle per stream is best up to a few GB of
+        // KV (every extra cut adds parts to the in-launch merges: 4 sequences x 128k keys run at 0.95 of the HBM
+        // roofline with 1 bundle per worker and 0.57 with 4); from ~16 GB on a launch lasts milliseconds and a second,
+        // queue-drawn bundle per worker evens out unequal stream rates (C5: -5 %).  Mixed launches: 2 per worker.
         const double kv_bytes = (double)total_blocks * kBlock * D * 2 * 2;
-        const double part_bytes = (double)G * D * 4 * 2;
-        int k = (int)std::floor(0.01 * kv_bytes / ((double)W * part_bytes));
-        k = std::max(mixed ? 2 : 1, std::min(4, k));      // measured on C2: 2 per worker beats 1, 3 and 4 in mixed launches
+        int k = (mixed || kv_bytes >= 16e9) ? 2 : 1;
         k = std::max(1, std::min(4, env_int("PA_BUNDLE_K", k)));
         const int64_t min_blocks = std::max(1, env_int("PA_MIN_BUNDLE_BLOCKS", 2));
         const int64_t target = std::max(min_blocks, (total_blocks + W * k - 1) / (W * k));

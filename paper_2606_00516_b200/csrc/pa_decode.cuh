@@ -212,29 +212,46 @@ __device__ __forceinline__ void decode_merge(const AttnParams& p, const DecItem&
     for (int h = 0; h < GG; ++h)
 #pragma unroll
         for (int k = 0; k < VPL; ++k) acc[h][k] = 0.f;
+    // PB parts' partial outputs are fetched together (as many as the register budget allows) and the (m, l) of
+    // the next four parts are already in flight, so a group of n parts costs ~n/PB + n/4 L2 round trips
+    constexpr int PB = (GG * VPL <= 16) ? 2 : 1;     // inlined in the consumer: keep within its register budget
+    float2 ml_next = make_float2(-INFINITY, 0.f);
+    if (pi < np) ml_next = __ldcg(ml_base + pi * kMaxGroup + hl);
     for (int c0 = 0; c0 < np; c0 += 4) {
+        const float2 ml = ml_next;
+        if (c0 + 4 + pi < np) ml_next = __ldcg(ml_base + (c0 + 4 + pi) * kMaxGroup + hl);
         float w = 0.f;
         if (c0 + pi < np) {
-            const float2 ml = __ldcg(ml_base + (c0 + pi) * kMaxGroup + hl);
             w = fast_exp2(ml.x - M);
             L += ml.y * w;
         }
         const int nk = min(4, np - c0);
-        for (int k = 0; k < nk; ++k) {
-            const float* src = pl.part_o + (int64_t)(ci.part_base + c0 + k) * G * D + lane * VPL;
-            float4 v[GG][VPL / 4];
 #pragma unroll
-            for (int h = 0; h < GG; ++h)
+        for (int k0 = 0; k0 < 4; k0 += PB) {
+            if (k0 < nk) {
+                float4 v[PB][GG][VPL / 4];
 #pragma unroll
-                for (int x = 0; x < VPL / 4; ++x)
-                    v[h][x] = __ldcg(reinterpret_cast<const float4*>(src + min(h, G - 1) * D) + x);
+                for (int kk = 0; kk < PB; ++kk) {
+                    const int part = ci.part_base + c0 + min(k0 + kk, nk - 1);      // clamped duplicate past the end
+                    const float* src = pl.part_o + (int64_t)part * G * D + lane * VPL;
 #pragma unroll
-            for (int h = 0; h < GG; ++h) {
-                const float wk = __shfl_sync(0xffffffffu, w, k * 8 + h);
+                    for (int h = 0; h < GG; ++h)
 #pragma unroll
-                for (int x = 0; x < VPL / 4; ++x) {
-                    acc[h][4 * x] += wk * v[h][x].x; acc[h][4 * x + 1] += wk * v[h][x].y;
-                    acc[h][4 * x + 2] += wk * v[h][x].z; acc[h][4 * x + 3] += wk * v[h][x].w;
+                        for (int x = 0; x < VPL / 4; ++x)
+                            v[kk][h][x] = __ldcg(reinterpret_cast<const float4*>(src + min(h, G - 1) * D) + x);
+                }
+#pragma unroll
+                for (int kk = 0; kk < PB; ++kk) {
+#pragma unroll
+                    for (int h = 0; h < GG; ++h) {
+                        float wk = __shfl_sync(0xffffffffu, w, (k0 + kk) * 8 + h);
+                        if (k0 + kk >= nk) wk = 0.f;
+#pragma unroll
+                        for (int x = 0; x < VPL / 4; ++x) {
+                            acc[h][4 * x] += wk * v[kk][h][x].x; acc[h][4 * x + 1] += wk * v[kk][h][x].y;
+                            acc[h][4 * x + 2] += wk * v[kk][h][x].z; acc[h][4 * x + 3] += wk * v[kk][h][x].w;
+                        }
+                    }
                 }
             }
         }
