@@ -290,7 +290,8 @@ def run_ours(args):
         graph, launch_mode = None, "eager"
         try:
             graph = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(graph):
+            # thread_local: the NCCL watchdog / NVML sampler threads neither break nor are broken by the capture
+            with torch.cuda.graph(graph, capture_error_mode="thread_local"):
                 for p in preps:
                     p.step()
             graph.replay()
