@@ -45,7 +45,8 @@ def _load():
     if _lib is None:
         _lib = C.CDLL(build())
         for name in ("oracle_kv_append", "oracle_kv_gather", "oracle_attention_rows", "oracle_attention_weights",
-                     "oracle_attention_partial", "oracle_merge", "oracle_fit", "oracle_quadratic_kappa"):
+                     "oracle_attention_partial", "oracle_merge", "oracle_fit", "oracle_quadratic_kappa", "oracle_theta0",
+                     "oracle_eq7"):
             getattr(_lib, name).restype = C.c_int32
     return _lib
 
@@ -192,3 +193,22 @@ def quadratic_kappa(r, K):
     if rc != 0:
         raise ValueError(f"oracle_quadratic_kappa: rc={rc}")
     return c, kappa.value
+
+
+def theta0(x: float):
+    """Base CFR threshold θ0 and ζ = −ln(1−θ0) from θ0/(1−θ0) + ln(1−θ0) = x, x = p0·α_p/α_d (Eq. 3)."""
+    th, ze = C.c_double(), C.c_double()
+    rc = _load().oracle_theta0(C.c_double(x), C.byref(th), C.byref(ze))
+    if rc != 0:
+        raise ValueError(f"oracle_theta0: rc={rc}")
+    return th.value, ze.value
+
+
+def eq7(alpha_p, beta_p, alpha_d, beta_d, alpha_mb, beta_mb_e, mu_L, mu_O, zeta, k0, N):
+    """Crossover condition (Eq. 7, Prop. 3.4) → dict(lhs, rhs, beta_eb_w, tp_eb, tp_mb)."""
+    out = [C.c_double() for _ in range(5)]
+    rc = _load().oracle_eq7(*[C.c_double(float(v)) for v in (alpha_p, beta_p, alpha_d, beta_d, alpha_mb, beta_mb_e,
+                                                               mu_L, mu_O, zeta, k0, N)], *[C.byref(o) for o in out])
+    if rc != 0:
+        raise ValueError(f"oracle_eq7: rc={rc}")
+    return dict(zip(("lhs", "rhs", "beta_eb_w", "tp_eb", "tp_mb"), (o.value for o in out)))

@@ -28,8 +28,9 @@
  *     pool[block][kv_head][slot_in_block][d],  bf16, C order,
  * and slot(s, t) = (block_tables[s][t / b], t % b).
  *
- * Parity pins: every function here is pinned by tests/test_oracle_pins.py (P1-P15) — nothing
- * is "parity unpinned".
+ * Parity pins: every function here is pinned by tests/test_oracle_pins.py (P1-P15; oracle_theta0 and
+ * oracle_eq7 by the hand-worked golden tests/golden/eq7_closed_forms.txt, the Eq. 3 residual and the
+ * throughput identity of Proposition 3.4) — nothing is "parity unpinned".
  *
  * Threading (pthread) only distributes independent (token row, q head) items to host cores for
  * the timed cpu_baseline; each item is computed by the plain loop in attend_row_head().
@@ -321,5 +322,46 @@ int32_t oracle_quadratic_kappa(const double* r, const double* K, int32_t count, 
         c[col] = dc / det;
     }
     *kappa = 2.0 * c[2] / (c[0] + c[1] + c[2]);
+    return 0;
+}
+
+/* Base threshold under CFR (§3.2.1, Proposition 3.1, Eq. 3): theta0 is the unique
+ * solution in (0, 1) of
+ *     theta0 / (1 - theta0) + ln(1 - theta0) = x,        x = p0 * alpha_p / alpha_d > 0,
+ * and zeta = -ln(1 - theta0).  The left side is 0 at theta0 = 0, increasing (derivative
+ * theta0 / (1 - theta0)^2 > 0) and unbounded as theta0 -> 1, so plain bisection on (0, 1) finds it.
+ * Returns -1 for x <= 0 or non-finite x. */
+int32_t oracle_theta0(double x, double* theta0, double* zeta) {
+    if (!(x > 0.0) || !isfinite(x)) return -1;
+    double lo = 0.0, hi = 1.0;
+    for (int it = 0; it < 200; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (mid <= lo || mid >= hi) break;
+        double f = mid / (1.0 - mid) + log(1.0 - mid) - x;
+        if (f < 0.0) lo = mid; else hi = mid;
+    }
+    *theta0 = 0.5 * (lo + hi);
+    *zeta = -log(1.0 - *theta0);
+    return 0;
+}
+
+/* Crossover condition, Proposition 3.4 / Eq. 7 (§3.5):  TP_MB(N) > TP_EB(k0*, N)  iff
+ *     beta_MB^e - beta_EB^w  <  1/(mu_L + mu_O) * [ (alpha_p + alpha_d zeta mu_O) / k0*  -  alpha_MB (1 + mu_O) / N ],
+ * with beta_EB^w = (beta_p mu_L + beta_d mu_O) / (mu_L + mu_O)  (below the TP_EB formula).
+ * Outputs: lhs (the marginal-cost gap), rhs (the amortised fixed-cost advantage of MB), beta_EB^w, and the two
+ * throughputs the proposition compares, written out from their own formulas:
+ *     TP_EB(k0*, N) = [ (alpha_p + alpha_d zeta mu_O) / k0*  +  beta_EB^w (mu_L + mu_O) ]^-1      (Eq. 4)
+ *     TP_MB(N)      = [ alpha_MB (1 + mu_O) / N  +  beta_MB^e (mu_L + mu_O) ]^-1
+ * Returns -1 unless mu_L + mu_O > 0, k0 > 0, N > 0. */
+int32_t oracle_eq7(double alpha_p, double beta_p, double alpha_d, double beta_d, double alpha_mb, double beta_mb_e,
+                   double mu_L, double mu_O, double zeta, double k0, double N,
+                   double* lhs, double* rhs, double* beta_eb_w, double* tp_eb, double* tp_mb) {
+    if (!(mu_L + mu_O > 0.0) || !(k0 > 0.0) || !(N > 0.0)) return -1;
+    double bw = (beta_p * mu_L + beta_d * mu_O) / (mu_L + mu_O);
+    *beta_eb_w = bw;
+    *lhs = beta_mb_e - bw;
+    *rhs = ((alpha_p + alpha_d * zeta * mu_O) / k0 - alpha_mb * (1.0 + mu_O) / N) / (mu_L + mu_O);
+    *tp_eb = 1.0 / ((alpha_p + alpha_d * zeta * mu_O) / k0 + bw * (mu_L + mu_O));
+    *tp_mb = 1.0 / (alpha_mb * (1.0 + mu_O) / N + beta_mb_e * (mu_L + mu_O));
     return 0;
 }

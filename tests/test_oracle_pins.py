@@ -373,3 +373,66 @@ def test_kappa_exact_quadratic_and_eq10():
     assert abs(kappa - 2 * c2 / (c0 + c1 + c2)) < 1e-11          # Eq. 11
     Kbar = (1 - r) * K[0] + r * K[-1]
     np.testing.assert_allclose(K - Kbar, -c[2] * r * (1 - r), atol=1e-11)   # Eq. 10
+
+
+def test_kappa_literal_value():
+    """K(r) = 2 + 5 r - 3 r^2: K(1) = 4, kappa = 2·(-3)/4 = -1.5 (Eq. 11), as a literal."""
+    r = np.linspace(0, 1, 11)
+    _, kappa = oracle.quadratic_kappa(r, 2 + 5 * r - 3 * r * r)
+    assert abs(kappa - (-1.5)) < 1e-11
+
+
+# ------------------------------------------------------------------ N3: Eq. 3 (theta0) and Eq. 7 (crossover)
+def test_eq7_golden_hand_worked():
+    g = _read_golden("eq7_closed_forms.txt")
+    o = oracle.eq7(*g["params"])
+    assert abs(o["beta_eb_w"] - g["beta_eb_w"][0]) < 1e-15
+    assert abs(o["lhs"] - g["lhs"][0]) < 1e-15 and abs(o["rhs"] - g["rhs"][0]) < 1e-15
+    assert abs(1 / o["tp_eb"] - g["inv_tp_eb"][0]) < 1e-12 and abs(1 / o["tp_mb"] - g["inv_tp_mb"][0]) < 1e-12
+    assert o["lhs"] > o["rhs"] and o["tp_mb"] < o["tp_eb"]
+
+
+def test_eq7_is_the_throughput_comparison_of_prop_3_4():
+    """Proposition 3.4: TP_MB > TP_EB  iff  LHS < RHS.  Algebraically 1/TP_MB - 1/TP_EB = (mu_L + mu_O)(LHS - RHS);
+    checked on random parameter draws, so a dropped term, a swapped mu or a wrong sign on either side breaks it."""
+    rng = np.random.default_rng(77)
+    flips = 0
+    for _ in range(400):
+        ap, ad, amb = rng.uniform(1e-4, 5e-2, 3)
+        bp, bd = rng.uniform(1e-6, 1e-4, 2)
+        bmb = rng.uniform(0.5, 1.5) * (bp + bd) / 2
+        muL, muO = rng.uniform(1, 3000), rng.uniform(1, 3000)
+        N = rng.integers(8, 4096)
+        th = rng.uniform(0.05, 0.95)
+        k0, zeta = max(1.0, np.floor(th * N)), -np.log(1 - th)
+        o = oracle.eq7(ap, bp, ad, bd, amb, bmb, muL, muO, zeta, k0, N)
+        d_inv = 1 / o["tp_mb"] - 1 / o["tp_eb"]
+        assert abs(d_inv - (muL + muO) * (o["lhs"] - o["rhs"])) < 1e-12 * max(1.0, abs(1 / o["tp_eb"]))
+        assert (o["tp_mb"] > o["tp_eb"]) == (o["lhs"] < o["rhs"])
+        flips += o["lhs"] < o["rhs"]
+        # beta_EB^w is a weighted average of beta_p and beta_d, and equals either one when the other weight is 0
+        assert min(bp, bd) - 1e-18 <= o["beta_eb_w"] <= max(bp, bd) + 1e-18
+    assert 20 < flips < 380                                   # both regimes occur in the sample
+    assert abs(oracle.eq7(1, 3e-5, 1, 7e-5, 1, 0, 10, 0, 1, 1, 1)["beta_eb_w"] - 3e-5) < 1e-20
+    assert abs(oracle.eq7(1, 3e-5, 1, 7e-5, 1, 0, 0, 10, 1, 1, 1)["beta_eb_w"] - 7e-5) < 1e-20
+    with pytest.raises(ValueError):
+        oracle.eq7(1, 1, 1, 1, 1, 1, 0, 0, 1, 1, 1)
+
+
+def test_theta0_golden_and_residual():
+    g = _read_golden("eq7_closed_forms.txt")
+    for x, th, ze in zip(g["theta0_x"], g["theta0_value"], g["theta0_zeta"]):
+        t, z = oracle.theta0(x)
+        assert abs(t - th) < 1e-12 and abs(z - ze) < 1e-12
+    # Proposition 3.1: theta0 depends only on x = p0 alpha_p / alpha_d, is increasing in it, and solves Eq. 3
+    prev = 0.0
+    for x in [1e-6, 1e-3, 0.05, 0.3, 1.0, 7.0, 100.0]:
+        t, z = oracle.theta0(x)
+        assert 0 < t < 1 and t > prev
+        assert abs(t / (1 - t) + np.log(1 - t) - x) < 1e-9 * max(1.0, x)
+        assert abs(z + np.log(1 - t)) < 1e-12
+        prev = t
+    # small-x asymptote: theta^2/2 + O(theta^3) = x  ->  theta0 ~ sqrt(2x)
+    assert abs(oracle.theta0(1e-8)[0] / np.sqrt(2e-8) - 1) < 1e-3
+    with pytest.raises(ValueError):
+        oracle.theta0(0.0)
