@@ -23,8 +23,17 @@
  *     the caller (PyTorch in this repo) owns pools, workspace, inputs and outputs.
  *   - bf16 tensors are dense, C order, 16-byte aligned base.  int32 index arrays are dense.
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All device work
- *     is enqueued on it; no call synchronises the device except pa_timer_end (on its own events)
- *     and pa_plan (which may wait for the previous plan's upload before reusing pinned staging).
+ *     is enqueued on it; no call synchronises the device except pa_timer_end (on its own events).
+ *     pa_plan stages its lists in a small ring of pinned host buffers and only waits (on an event of
+ *     its own) when the buffer it is about to reuse still has an upload in flight, i.e. when more
+ *     than 3 plans are outstanding on the device.  pa_kv_append, pa_batch_attention and pa_kv_gather only
+ *     enqueue kernels and may be captured into a CUDA graph; pa_plan (a host-to-device upload from
+ *     library-owned staging) and the pa_timer_* calls must NOT be called during stream capture.
+ *   - The CUDA device current on the calling thread must be cfg.device for every call that takes a
+ *     stream (PA_ERR_INVALID otherwise).  pa_create restores the caller's current device before it
+ *     returns.  A context is not thread-safe: one thread at a time per pa_ctx; different contexts
+ *     (also on different devices) may be used concurrently.
+ *   - No environment variable is read.  Every tuning knob is a field of pa_config.
  *   - Return value: PA_OK or a negative PA_ERR_*; pa_last_error(ctx) gives a message.  No
  *     exceptions, no aborts, no printing.  Out-of-range block ids inside block tables are
  *     undefined behaviour (not validated on the device).
@@ -60,7 +69,8 @@ extern "C" {
 #define PA_ERR_TIMER (-5)       /* fewer than 2 distinct n_tok recorded for that r */
 
 /* flags for pa_config.flags */
-#define PA_FLAG_DEBUG_SIMPLE 1u /* debug: route every row through the plain one-warp-per-(row,head) CUDA kernel */
+#define PA_FLAG_DEBUG_SIMPLE 1u   /* debug: route every row through the plain one-warp-per-(row,head) CUDA kernel */
+#define PA_FLAG_PREFILL_P_SMEM 2u /* prefill variant that stages P in shared memory instead of TMEM (default: TMEM) */
 
 typedef struct pa_ctx pa_ctx; /* opaque; owns host plan scratch, pinned staging, CUDA events, timer samples */
 
@@ -75,6 +85,11 @@ typedef struct {
     int32_t max_blocks_per_seq; /* row stride of block_tables (entries) */
     int32_t device;             /* CUDA device ordinal */
     uint32_t flags;             /* PA_FLAG_* */
+    /* planner tuning; 0 = the planner's own choice.  Effective values: pa_plan_info 6, 7. */
+    int32_t tune_prefill_ctas;        /* CTAs that start in the prefill role of a mixed launch (clamped to [1, SMs-1]) */
+    int32_t tune_bundles_per_stream;  /* decode bundles per persistent stream, 1..4 */
+    int32_t tune_min_bundle_blocks;   /* smallest decode bundle, in 16-token blocks (default 2) */
+    int32_t reserved;                 /* must be 0 */
 } pa_config;
 
 /* Create / destroy a context for one shape.  `out` host.  PA_ERR_UNSUPPORTED for shapes outside the
@@ -117,6 +132,10 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu_seqlens_q, const int32_t* h_con
  *     t = 0 .. context_lens[s] + j,   K_s/V_s read from the pools through block_tables,
  * bf16 inputs, fp32 accumulation, bf16 output rounded once.  Uses the last pa_plan of ctx; the
  * device descriptor arrays must describe the same batch as the planned host copies.
+ * Range: any finite bf16 inputs.  The tensor-core prefill path exponentiates a 128-key tile against the running
+ * maximum of the EARLIER tiles of the row; a row in which one tile's scores exceed everything before them by more
+ * than 2^127 (88 nats) overflows that pass, is detected (its row sum is not finite) and is recomputed in the same
+ * launch by a plain two-pass loop, so the result is the general softmax for such rows too (just slower).
  *   q    dev bf16 [n_tok, Hq, D] (read);  out dev bf16 [n_tok, Hq, D] (every planned row written)
  *   k_pool, v_pool dev bf16 pools (read only).
  * Decode rows run the split-KV path (partials in the workspace, merged in the same launch by the
@@ -149,10 +168,23 @@ int32_t pa_timer_fit(pa_ctx* ctx, double r, double* alpha, double* beta, double*
 int32_t pa_timer_kappa(pa_ctx* ctx, int32_t n_tok, double* c, double* kappa, int32_t* n_points);
 int32_t pa_timer_reset(pa_ctx* ctx);
 
+/* N3 (Prop. 3.1 Eq. 3-4, L184-191 Prop. 3.4 Eq. 7): scalar host arithmetic (fp64)
+ * on fitted coefficients; no device work, ctx may be NULL.
+ * pa_crossover_theta0: the base CFR threshold theta0 in (0,1) solving theta0/(1-theta0) + ln(1-theta0) = x with
+ *   x = p0*alpha_p/alpha_d > 0, and zeta = -ln(1-theta0).  PA_ERR_INVALID for x <= 0 or non-finite.
+ * pa_crossover_eq7: in[11] = {alpha_p, beta_p, alpha_d, beta_d, alpha_MB, beta_MB^e, mu_L, mu_O, zeta, k0*, N};
+ *   out[5] = {LHS = beta_MB^e - beta_EB^w,  RHS = [(alpha_p + alpha_d zeta mu_O)/k0* - alpha_MB(1+mu_O)/N]/(mu_L+mu_O),
+ *             beta_EB^w = (beta_p mu_L + beta_d mu_O)/(mu_L+mu_O),  TP_EB(k0*, N) (Eq. 4),  TP_MB(N)}.
+ *   Mixed batching wins iff LHS < RHS.  PA_ERR_INVALID unless mu_L + mu_O > 0, k0* > 0, N > 0. */
+int32_t pa_crossover_theta0(double x, double* theta0, double* zeta);
+int32_t pa_crossover_eq7(const double* in, double* out);
+
 /* Introspection of the last plan (host ints; for bench.py's launch accounting and the tests).
  * which: 0 decode work items, 1 decode bundles, 2 split (partial-writing) items, 3 prefill tiles,
  *        4 CTAs in the attention launch, 5 kernel launches per pa_batch_attention call,
- *        6 CTAs given the prefill role in the mixed launch. */
+ *        6 CTAs given the prefill role in the mixed launch, 7 decode bundles per stream (effective),
+ *        8 prefill variant (0 P in TMEM, 1 P in shared memory, 2 plain kernel),
+ *        9 host nanoseconds the last pa_plan call took (validation + lists + enqueue of the upload). */
 int64_t pa_plan_info(const pa_ctx* ctx, int32_t which);
 
 /* Library-owned message of the last error on ctx (valid until the next call on ctx); "" if none. */

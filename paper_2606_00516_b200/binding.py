@@ -17,10 +17,12 @@ LIB_PATH = os.path.join(_HERE, "libpa_b200.so")
 PA_OK = 0
 PA_ERR_INVALID, PA_ERR_UNSUPPORTED, PA_ERR_WORKSPACE, PA_ERR_CUDA, PA_ERR_TIMER = -1, -2, -3, -4, -5
 PA_FLAG_DEBUG_SIMPLE = 1
+PA_FLAG_PREFILL_P_SMEM = 2
 
 EXPORTS = ["pa_create", "pa_destroy", "pa_workspace_bytes", "pa_kv_pool_bytes", "pa_kv_append", "pa_plan",
            "pa_batch_attention", "pa_kv_gather", "pa_timer_begin", "pa_timer_end", "pa_timer_record",
-           "pa_timer_fit", "pa_timer_kappa", "pa_timer_reset", "pa_plan_info", "pa_last_error"]
+           "pa_timer_fit", "pa_timer_kappa", "pa_timer_reset", "pa_crossover_theta0", "pa_crossover_eq7", "pa_plan_info",
+           "pa_last_error"]
 
 
 class PaError(RuntimeError):
@@ -33,7 +35,8 @@ class PaConfig(C.Structure):
     _fields_ = [("num_q_heads", C.c_int32), ("num_kv_heads", C.c_int32), ("head_dim", C.c_int32),
                 ("block_size", C.c_int32), ("num_blocks", C.c_int64), ("max_seqs", C.c_int32),
                 ("max_tokens", C.c_int32), ("max_blocks_per_seq", C.c_int32), ("device", C.c_int32),
-                ("flags", C.c_uint32)]
+                ("flags", C.c_uint32), ("tune_prefill_ctas", C.c_int32), ("tune_bundles_per_stream", C.c_int32),
+                ("tune_min_bundle_blocks", C.c_int32), ("reserved", C.c_int32)]
 
 
 _lib = None
@@ -64,6 +67,8 @@ def load_library() -> C.CDLL:
         lib.pa_timer_fit.argtypes = [vp, f64, C.POINTER(f64), C.POINTER(f64), C.POINTER(f64), C.POINTER(i32)]
         lib.pa_timer_kappa.argtypes = [vp, i32, C.POINTER(f64), C.POINTER(f64), C.POINTER(i32)]
         lib.pa_timer_reset.argtypes = [vp]
+        lib.pa_crossover_theta0.argtypes = [f64, C.POINTER(f64), C.POINTER(f64)]
+        lib.pa_crossover_eq7.argtypes = [C.POINTER(f64), C.POINTER(f64)]
         lib.pa_plan_info.argtypes = [vp, i32]
         lib.pa_plan_info.restype = i64
         lib.pa_last_error.argtypes = [vp]
@@ -79,6 +84,17 @@ def _ptr(t) -> int:
     return 0 if t is None else t.data_ptr()
 
 
+def _host_i32(a) -> int:
+    """Address of a HOST int32 array (kept alive by the caller for the duration of the call)."""
+    import numpy as np
+    if isinstance(a, np.ndarray) and a.dtype == np.int32 and a.flags.c_contiguous:
+        return a.ctypes.data
+    t = torch.as_tensor(a, dtype=torch.int32).contiguous()
+    assert t.device.type == "cpu"
+    _host_i32.keep = t          # survives until the next conversion, i.e. past the C call that uses the address
+    return t.data_ptr()
+
+
 def _stream(stream) -> int:
     if stream is None:
         stream = torch.cuda.current_stream()
@@ -89,10 +105,12 @@ class PagedAttention:
     """One context per shape.  Methods mirror the C entry points one to one."""
 
     def __init__(self, num_q_heads: int, num_kv_heads: int, head_dim: int, num_blocks: int, max_seqs: int,
-                 max_tokens: int, max_blocks_per_seq: int, block_size: int = 16, device: int = 0, flags: int = 0):
+                 max_tokens: int, max_blocks_per_seq: int, block_size: int = 16, device: int = 0, flags: int = 0,
+                 tune_prefill_ctas: int = 0, tune_bundles_per_stream: int = 0, tune_min_bundle_blocks: int = 0):
         self.lib = load_library()
         self.cfg = PaConfig(num_q_heads, num_kv_heads, head_dim, block_size, num_blocks, max_seqs, max_tokens,
-                            max_blocks_per_seq, device, flags)
+                            max_blocks_per_seq, device, flags, tune_prefill_ctas, tune_bundles_per_stream,
+                            tune_min_bundle_blocks, 0)
         self.ctx = C.c_void_p()
         rc = self.lib.pa_create(C.byref(self.ctx), C.byref(self.cfg))
         if rc != PA_OK:
@@ -135,12 +153,10 @@ class PagedAttention:
                                           _stream(stream)))
 
     def plan(self, h_cu_seqlens_q, h_context_lens, n_seq: int, num_decode_seqs: int, stream=None):
-        """h_* are HOST int32 tensors/arrays (numpy or CPU torch)."""
-        cu = torch.as_tensor(h_cu_seqlens_q, dtype=torch.int32).contiguous()
-        cl = torch.as_tensor(h_context_lens, dtype=torch.int32).contiguous()
-        assert cu.device.type == "cpu" and cl.device.type == "cpu"
-        self._check(self.lib.pa_plan(self.ctx, cu.data_ptr(), cl.data_ptr(), n_seq, num_decode_seqs,
-                                     self.workspace.data_ptr(), self.workspace.numel(), _stream(stream)))
+        """h_* are HOST int32 arrays: contiguous numpy int32 (passed as they are) or anything torch.as_tensor takes."""
+        self._check(self.lib.pa_plan(self.ctx, _host_i32(h_cu_seqlens_q), _host_i32(h_context_lens), n_seq,
+                                     num_decode_seqs, self.workspace.data_ptr(), self.workspace.numel(),
+                                     _stream(stream)))
 
     def batch_attention(self, q, k_pool, v_pool, cu_seqlens_q, context_lens, block_tables, softmax_scale: float, out,
                         stream=None):
@@ -173,6 +189,23 @@ class PagedAttention:
         c, k, n = (C.c_double * 3)(), C.c_double(), C.c_int32()
         self._check(self.lib.pa_timer_kappa(self.ctx, n_tok, c, C.byref(k), C.byref(n)))
         return (c[0], c[1], c[2]), k.value, n.value
+
+    def crossover_theta0(self, x: float):
+        """(theta0, zeta) of PAPER.md Eq. 3 for x = p0·alpha_p/alpha_d."""
+        th, ze = C.c_double(), C.c_double()
+        rc = self.lib.pa_crossover_theta0(x, C.byref(th), C.byref(ze))
+        if rc != PA_OK:
+            raise PaError(rc, "pa_crossover_theta0: x must be positive and finite")
+        return th.value, ze.value
+
+    def crossover_eq7(self, alpha_p, beta_p, alpha_d, beta_d, alpha_mb, beta_mb_e, mu_L, mu_O, zeta, k0, N):
+        """PAPER.md Eq. 7 → dict(lhs, rhs, beta_eb_w, tp_eb, tp_mb); mixed batching wins iff lhs < rhs."""
+        a = (C.c_double * 11)(alpha_p, beta_p, alpha_d, beta_d, alpha_mb, beta_mb_e, mu_L, mu_O, zeta, k0, N)
+        o = (C.c_double * 5)()
+        rc = self.lib.pa_crossover_eq7(a, o)
+        if rc != PA_OK:
+            raise PaError(rc, "pa_crossover_eq7: needs mu_L + mu_O > 0, k0 > 0, N > 0")
+        return dict(zip(("lhs", "rhs", "beta_eb_w", "tp_eb", "tp_mb"), list(o)))
 
     def timer_reset(self):
         self._check(self.lib.pa_timer_reset(self.ctx))

@@ -1,11 +1,13 @@
 // C-ABI layer of libpa_b200.so (include/pa.h): context, validation, planner (a1/a7), launches, timer (a8).
 // Host code only; kernels live in pa_kernels.cu.
 #include <algorithm>
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -20,18 +22,21 @@ struct pa_ctx {
     int num_sms = 0;
     std::string err;
     // workspace layout (bytes from the workspace base)
-    int64_t off_counters = 0, off_plan = 0, off_part_ml = 0, off_part_o = 0, ws_bytes = 0;
+    int64_t off_counters = 0, off_plan = 0, off_redo = 0, off_part_ml = 0, off_part_o = 0, ws_bytes = 0;
     int64_t plan_region_bytes = 0;
-    int32_t max_items = 0, max_bundles = 0, max_tiles = 0, max_split = 0, max_workers = 0;
-    // pinned staging for the plan upload
-    uint8_t* h_stage = nullptr;
-    cudaEvent_t stage_ev = nullptr;
-    bool stage_pending = false;
+    int32_t max_bundles = 0, max_tiles = 0, max_split = 0, max_workers = 0;
+    // pinned staging for the plan upload: a ring, so that pa_plan only waits when kStages plans are in flight
+    static constexpr int kStages = 3;
+    uint8_t* h_stage[kStages] = {nullptr, nullptr, nullptr};
+    cudaEvent_t stage_ev[kStages] = {nullptr, nullptr, nullptr};
+    bool stage_pending[kStages] = {false, false, false};
+    int stage_next = 0;
     // current plan
     bool planned = false;
     PlanView view{};
     int32_t decode_ctas = 0, n_simple_tiles = 0, launches_per_call = 0, prefill_ctas = 0, p_in_tmem = 1;
-    int32_t planned_n_tok = 0;
+    int32_t planned_n_tok = 0, n_items = 0, bundles_per_stream = 0, prefill_mode = 0;
+    int64_t plan_host_ns = 0;
     // tensor-map cache
     const void* tm_k_ptr = nullptr;
     const void* tm_v_ptr = nullptr;
@@ -51,8 +56,8 @@ namespace {
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-EncodeTiledFn g_encode = nullptr;
-bool g_configured = false;
+EncodeTiledFn g_encode = nullptr;      // driver entry point, resolved once per process (std::call_once)
+std::once_flag g_encode_once;
 
 int32_t fail(pa_ctx* ctx, int32_t code, const std::string& msg) {
     if (ctx) ctx->err = msg;
@@ -63,21 +68,31 @@ int32_t cuda_fail(pa_ctx* ctx, cudaError_t e, const char* where) {
 }
 int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
-int env_int(const char* name, int dflt) {
-    const char* v = std::getenv(name);
-    return v && *v ? std::atoi(v) : dflt;
+// every call that enqueues work requires cfg.device to be the calling thread's current device
+int32_t check_device(pa_ctx* ctx, const char* where) {
+    int cur = -1;
+    cudaError_t e = cudaGetDevice(&cur);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, where);
+    if (cur != ctx->cfg.device)
+        return fail(ctx, PA_ERR_INVALID, std::string(where) + ": current CUDA device " + std::to_string(cur) +
+                                             " is not the context's device " + std::to_string(ctx->cfg.device));
+    return PA_OK;
+}
+
+bool resolve_encode() {
+    std::call_once(g_encode_once, [] {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess && fn)
+            g_encode = reinterpret_cast<EncodeTiledFn>(fn);
+    });
+    return g_encode != nullptr;
 }
 
 // pool[num_blocks][Hkv][16][D] bf16 -> 4-D tensor map, box = 64 columns x 16 tokens of one (block, head), 128B swizzle
 // rows < 16: the same tensor with a shorter box, used to fetch only the filled rows of a sequence's last block
 int32_t make_pool_map(pa_ctx* ctx, const void* pool, CUtensorMap* out, int rows = kBlock) {
-    if (!g_encode) {
-        void* fn = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
-        if (e != cudaSuccess || !fn) return fail(ctx, PA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
-        g_encode = reinterpret_cast<EncodeTiledFn>(fn);
-    }
+    if (!resolve_encode()) return fail(ctx, PA_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
     const pa_config& c = ctx->cfg;
     const cuuint64_t D = c.head_dim, Hkv = c.num_kv_heads;
     cuuint64_t dims[4] = {D, (cuuint64_t)kBlock, Hkv, (cuuint64_t)c.num_blocks};
@@ -152,11 +167,16 @@ int32_t pa_create(pa_ctx** out, const pa_config* cfg) {
     if (!out || !cfg) return PA_ERR_INVALID;
     *out = nullptr;
     if (cfg->num_q_heads <= 0 || cfg->num_kv_heads <= 0 || cfg->num_blocks <= 0 || cfg->max_seqs <= 0 ||
-        cfg->max_tokens <= 0 || cfg->max_blocks_per_seq <= 0 || cfg->device < 0)
+        cfg->max_tokens <= 0 || cfg->max_blocks_per_seq <= 0 || cfg->device < 0 || cfg->tune_prefill_ctas < 0 ||
+        cfg->tune_bundles_per_stream < 0 || cfg->tune_bundles_per_stream > 4 || cfg->tune_min_bundle_blocks < 0 ||
+        cfg->reserved != 0)
         return PA_ERR_INVALID;
     if ((cfg->head_dim != 128 && cfg->head_dim != 256) || cfg->block_size != kBlock ||
         cfg->num_q_heads % cfg->num_kv_heads != 0 || cfg->num_q_heads / cfg->num_kv_heads > kMaxGroup)
         return PA_ERR_UNSUPPORTED;
+    // the caller's current device is restored before returning (success or failure)
+    int prev_device = -1;
+    if (cudaGetDevice(&prev_device) != cudaSuccess) { cudaGetLastError(); return PA_ERR_CUDA; }
     pa_ctx* ctx = new pa_ctx();
     ctx->cfg = *cfg;
     ctx->G = cfg->num_q_heads / cfg->num_kv_heads;
@@ -164,53 +184,59 @@ int32_t pa_create(pa_ctx** out, const pa_config* cfg) {
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, cfg->device);
     int cc_major = 0;
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, cfg->device);
+    // opt-in shared memory is a per-device function attribute: set it for this context's device every time
+    if (e == cudaSuccess && cc_major == 10) e = configure_kernels();
     if (e != cudaSuccess || cc_major != 10) {
+        cudaGetLastError();
         delete ctx;
+        cudaSetDevice(prev_device);
         return PA_ERR_CUDA;  // no usable sm_100 device: there is no fallback path
-    }
-    if (!g_configured) {
-        e = configure_kernels();
-        if (e != cudaSuccess) { delete ctx; return PA_ERR_CUDA; }
-        g_configured = true;
     }
     // ---- workspace layout
     ctx->max_workers = ctx->num_sms * kDecodeWarps;
     // k <= 4 equal bundles per worker, plus the bundles that uncut short groups close early (at most one per group)
     const int32_t eq_bundles = ctx->max_workers * 5 + 8;
     ctx->max_bundles = eq_bundles + cfg->max_seqs * cfg->num_kv_heads;
-    ctx->max_items = cfg->max_seqs * cfg->num_kv_heads + ctx->max_bundles + 8;
     ctx->max_split = 2 * eq_bundles;          // only groups cut by a bundle boundary have partials
     ctx->max_tiles = cfg->max_tokens / kQTile + cfg->max_seqs + 1;
     int64_t off = 0;
     ctx->off_counters = off;
     off += align_up(16 * 4 + (int64_t)cfg->max_seqs * cfg->num_kv_heads * 4, 256);
     ctx->off_plan = off;
-    ctx->plan_region_bytes = align_up((int64_t)ctx->max_items * sizeof(DecItem), 256) +
-                             align_up((int64_t)(ctx->max_bundles + 1) * 4, 256) +
+    ctx->plan_region_bytes = align_up((int64_t)ctx->max_bundles * sizeof(DecBundle), 256) +
                              align_up((int64_t)ctx->max_tiles * sizeof(PreTile), 256);
     off += ctx->plan_region_bytes;
+    ctx->off_redo = off;
+    off += align_up((int64_t)cfg->max_tokens * cfg->num_q_heads * sizeof(int2), 256);
     ctx->off_part_ml = off;
     off += align_up((int64_t)ctx->max_split * kMaxGroup * sizeof(float2), 256);
     ctx->off_part_o = off;
     off += align_up((int64_t)ctx->max_split * ctx->G * cfg->head_dim * 4, 256);
     ctx->ws_bytes = off;
-    e = cudaMallocHost(reinterpret_cast<void**>(&ctx->h_stage), (size_t)ctx->plan_region_bytes);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->stage_ev, cudaEventDisableTiming);
+    for (int i = 0; i < pa_ctx::kStages && e == cudaSuccess; ++i) {
+        e = cudaMallocHost(reinterpret_cast<void**>(&ctx->h_stage[i]), (size_t)ctx->plan_region_bytes);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->stage_ev[i], cudaEventDisableTiming);
+    }
     if (e == cudaSuccess) e = cudaEventCreate(&ctx->t0);
     if (e == cudaSuccess) e = cudaEventCreate(&ctx->t1);
     if (e != cudaSuccess) {
+        cudaGetLastError();
         pa_destroy(ctx);
+        cudaSetDevice(prev_device);
         return PA_ERR_CUDA;
     }
+    cudaSetDevice(prev_device);
     *out = ctx;
     return PA_OK;
 }
 
 int32_t pa_destroy(pa_ctx* ctx) {
     if (!ctx) return PA_ERR_INVALID;
-    if (ctx->stage_pending && ctx->stage_ev) cudaEventSynchronize(ctx->stage_ev);
-    if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
-    if (ctx->stage_ev) cudaEventDestroy(ctx->stage_ev);
+    for (int i = 0; i < pa_ctx::kStages; ++i) {
+        if (ctx->stage_pending[i] && ctx->stage_ev[i]) cudaEventSynchronize(ctx->stage_ev[i]);
+        if (ctx->h_stage[i]) cudaFreeHost(ctx->h_stage[i]);
+        if (ctx->stage_ev[i]) cudaEventDestroy(ctx->stage_ev[i]);
+    }
     if (ctx->t0) cudaEventDestroy(ctx->t0);
     if (ctx->t1) cudaEventDestroy(ctx->t1);
     delete ctx;
@@ -236,6 +262,7 @@ int32_t pa_kv_append(pa_ctx* ctx, const void* k_new, const void* v_new, void* k_
         return fail(ctx, PA_ERR_INVALID, "pa_kv_append: null pointer");
     if (n_seq > ctx->cfg.max_seqs || n_tok > ctx->cfg.max_tokens)
         return fail(ctx, PA_ERR_INVALID, "pa_kv_append: n_seq/n_tok exceed the configured maxima");
+    if (int32_t rc = check_device(ctx, "pa_kv_append")) return rc;
     LaunchShape sh{ctx->cfg.num_q_heads, ctx->cfg.num_kv_heads, ctx->cfg.head_dim, ctx->cfg.max_blocks_per_seq};
     cudaError_t e = launch_kv_append(sh, k_new, v_new, k_pool, v_pool, d_cu, d_ctx, d_bt, n_seq, n_tok,
                                      static_cast<cudaStream_t>(stream));
@@ -250,20 +277,72 @@ int32_t pa_kv_gather(pa_ctx* ctx, const void* k_pool, const void* v_pool, const 
     if (!k_pool || !v_pool || !d_row || !k_out || !v_out) return fail(ctx, PA_ERR_INVALID, "pa_kv_gather: null pointer");
     if (kv_len > (int64_t)ctx->cfg.max_blocks_per_seq * kBlock)
         return fail(ctx, PA_ERR_INVALID, "pa_kv_gather: kv_len exceeds max_blocks_per_seq * 16");
+    if (int32_t rc = check_device(ctx, "pa_kv_gather")) return rc;
     LaunchShape sh{ctx->cfg.num_q_heads, ctx->cfg.num_kv_heads, ctx->cfg.head_dim, ctx->cfg.max_blocks_per_seq};
     cudaError_t e = launch_kv_gather(sh, k_pool, v_pool, d_row, kv_len, k_out, v_out, static_cast<cudaStream_t>(stream));
     return e == cudaSuccess ? PA_OK : cuda_fail(ctx, e, "pa_kv_gather");
 }
 
 // ---------------------------------------------------------------------------------------------
-// a1 plan.  Decode: the blocks of all (decode seq, KV head) groups form one stream that is cut into
-// equal-cost bundles (k per persistent worker; k grows with the batch so that the split partials stay
-// <= ~1 % of the KV bytes); a group cut by a bundle boundary becomes several items whose partials the
-// last-arriving worker merges.  Prefill: 128-row query tiles.
+// a1 plan.  Decode: the blocks of all (decode seq, KV head) groups form one stream (group order) that is cut into
+// equal-cost bundles; a group cut by a bundle boundary is a split group whose partials the last-arriving worker
+// merges.  The plan holds one 32-byte DecBundle per bundle (the streams derive their items from it and from
+// context_lens), so it is O(bundles + sequences) host work and a few KB of upload, not O(groups).
+// Prefill: 128-row query tiles in longest-first order.
 // ---------------------------------------------------------------------------------------------
+namespace {
+
+// Cuts the decode block stream into bundles, writing DecBundle records in place.
+struct BundleCutter {
+    DecBundle* out;
+    int32_t max_bundles, max_split;
+    int64_t target;
+    int32_t n_bundles = 0, n_split = 0, n_items = 0;
+    int64_t cur = 0;          // blocks in the open bundle (out[n_bundles])
+    bool open = false;
+    bool overflow = false;
+
+    void add(int32_t grp, int32_t b0, int32_t b1, int32_t nblk) {   // blocks [b0, b1) of group grp join the open bundle
+        if (n_bundles >= max_bundles) { overflow = true; return; }
+        DecBundle& d = out[n_bundles];
+        if (!open) {
+            d = DecBundle{grp, b0, grp, 0, -1, 1, -1, 1};
+            open = true;
+        }
+        d.grp_end = grp;
+        d.blk_end = b1 == nblk ? -1 : b1;
+        cur += b1 - b0;
+        ++n_items;
+    }
+    void add_whole_sequence(int32_t grp0, int32_t groups, int32_t nblk) {   // `groups` consecutive groups, uncut
+        add(grp0, 0, nblk, nblk);
+        if (overflow) return;
+        out[n_bundles].grp_end = grp0 + groups - 1;
+        n_items += groups - 1;
+        cur += (int64_t)(groups - 1) * nblk;
+    }
+    void close() {
+        if (open) { ++n_bundles; open = false; }
+        cur = 0;
+    }
+    // the group `grp` was emitted as `parts` consecutive parts, the first one into bundle `first_bundle`
+    void mark_split(int32_t grp, int32_t first_bundle, int32_t parts) {
+        if (n_split + parts > max_split || parts > 0xffff) { overflow = true; return; }
+        for (int32_t i = 0; i < parts; ++i) {
+            DecBundle& d = out[first_bundle + i];
+            if (d.grp_begin == grp) { d.first_part_base = n_split; d.first_part = (i << 16) | parts; }
+            else { d.last_part_base = n_split; d.last_part = (i << 16) | parts; }
+        }
+        n_split += parts;
+    }
+};
+
+}  // namespace
+
 int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t n_seq, int32_t num_decode_seqs,
                 void* d_workspace, int64_t workspace_bytes, void* stream_) {
     if (!ctx) return PA_ERR_INVALID;
+    const auto t_begin = std::chrono::steady_clock::now();
     ctx->planned = false;
     const pa_config& c = ctx->cfg;
     if (n_seq < 0 || num_decode_seqs < 0 || num_decode_seqs > n_seq)
@@ -273,48 +352,55 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     if (!d_workspace || workspace_bytes < ctx->ws_bytes || (reinterpret_cast<uintptr_t>(d_workspace) & 255))
         return fail(ctx, PA_ERR_WORKSPACE, "pa_plan: workspace missing, misaligned or smaller than pa_workspace_bytes");
     if (n_seq > 0 && h_cu[0] != 0) return fail(ctx, PA_ERR_INVALID, "pa_plan: cu_seqlens_q[0] != 0");
+    const int64_t max_kv = (int64_t)c.max_blocks_per_seq * kBlock;
+    int64_t total_blocks_1 = 0;     // blocks of the decode sequences, per KV head
     for (int s = 0; s < n_seq; ++s) {
         const int64_t ql = (int64_t)h_cu[s + 1] - h_cu[s];
         if (ql < 0) return fail(ctx, PA_ERR_INVALID, "pa_plan: cu_seqlens_q not non-decreasing");
         if (h_ctx[s] < 0) return fail(ctx, PA_ERR_INVALID, "pa_plan: negative context length");
-        if (s < num_decode_seqs && ql != 1) return fail(ctx, PA_ERR_INVALID, "pa_plan: decode sequence with q_len != 1");
-        if ((int64_t)h_ctx[s] + ql > (int64_t)c.max_blocks_per_seq * kBlock)
-            return fail(ctx, PA_ERR_INVALID, "pa_plan: kv_len exceeds max_blocks_per_seq * 16");
+        if (s < num_decode_seqs) {
+            if (ql != 1) return fail(ctx, PA_ERR_INVALID, "pa_plan: decode sequence with q_len != 1");
+            total_blocks_1 += ((int64_t)h_ctx[s] + kBlock) / kBlock;     // ceil((ctx + 1) / 16)
+        }
+        if ((int64_t)h_ctx[s] + ql > max_kv) return fail(ctx, PA_ERR_INVALID, "pa_plan: kv_len exceeds max_blocks_per_seq * 16");
     }
     const int32_t n_tok = n_seq > 0 ? h_cu[n_seq] : 0;
     if (n_tok > c.max_tokens) return fail(ctx, PA_ERR_INVALID, "pa_plan: n_tok > max_tokens");
+    if (int32_t rc = check_device(ctx, "pa_plan")) return rc;
 
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-    if (ctx->stage_pending) {
-        cudaError_t e = cudaEventSynchronize(ctx->stage_ev);
+    const int stage = ctx->stage_next;
+    if (ctx->stage_pending[stage]) {    // only when kStages plans are already in flight
+        cudaError_t e = cudaEventSynchronize(ctx->stage_ev[stage]);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "pa_plan(stage sync)");
-        ctx->stage_pending = false;
+        ctx->stage_pending[stage] = false;
     }
+    uint8_t* h_stage = ctx->h_stage[stage];
     const bool simple_all = (c.flags & PA_FLAG_DEBUG_SIMPLE) != 0;
     const int Hkv = c.num_kv_heads, D = c.head_dim, G = ctx->G;
 
-    // ---- prefill tiles (built first: the decode bundling below depends on how many CTAs prefill takes)
-    std::vector<PreTile> tile_vec;
+    // ---- prefill tiles (built first: the decode bundling below depends on how many CTAs prefill takes);
+    // staging layout: tiles | bundles
+    PreTile* tiles = reinterpret_cast<PreTile*>(h_stage);
+    int32_t n_tiles = 0;
     for (int s = simple_all ? 0 : num_decode_seqs; s < n_seq; ++s) {
         const int32_t ql = h_cu[s + 1] - h_cu[s];
         for (int32_t q0 = 0; q0 < ql; q0 += kQTile) {
-            if ((int32_t)tile_vec.size() >= ctx->max_tiles) return fail(ctx, PA_ERR_INVALID, "pa_plan: tile list overflow");
-            const int32_t rows = std::min(kQTile, ql - q0);
-            tile_vec.push_back(PreTile{s, q0, rows, h_ctx[s], h_ctx[s] + ql, h_cu[s], {0, 0}});
+            if (n_tiles >= ctx->max_tiles) return fail(ctx, PA_ERR_INVALID, "pa_plan: tile list overflow");
+            tiles[n_tiles++] = PreTile{s, q0, std::min(kQTile, ql - q0), h_ctx[s], h_ctx[s] + ql, h_cu[s], {0, 0}};
         }
     }
-    const int32_t n_tiles = (int32_t)tile_vec.size();
     // longest first: the queue then hands out units in LPT order (causal tiles late in a chunk see more keys)
-    std::stable_sort(tile_vec.begin(), tile_vec.end(), [](const PreTile& a, const PreTile& b) {
+    std::stable_sort(tiles, tiles + n_tiles, [](const PreTile& a, const PreTile& b) {
         return a.ctx + a.q_begin + a.q_rows > b.ctx + b.q_begin + b.q_rows;
     });
-    const int prefill_mode = simple_all ? 2 : env_int("PA_PREFILL_MODE", 0);   // 0 P in TMEM, 1 P in smem, 2 plain kernel
+    // prefill variant: 0 P in TMEM, 1 P in shared memory, 2 plain kernel
+    const int prefill_mode = simple_all ? 2 : ((c.flags & PA_FLAG_PREFILL_P_SMEM) ? 1 : 0);
     const int NQ = D == 128 ? 2 : 1;
     const int32_t head_groups = (G + NQ - 1) / NQ;
     const int32_t n_units = prefill_mode == 2 ? 0 : n_tiles * Hkv * head_groups;
     const int n_dec = simple_all ? 0 : num_decode_seqs;
-    int64_t total_blocks = 0;
-    for (int s = 0; s < n_dec; ++s) total_blocks += ((int64_t)h_ctx[s] + 1 + kBlock - 1) / kBlock * Hkv;
+    const int64_t total_blocks = n_dec > 0 ? total_blocks_1 * Hkv : 0;
     // ---- CTA partition of the single launch (a7): share the SMs in proportion to the CTA-time of the two roles,
     // from rates measured with per-CTA timestamps on B200.  Prefill: ~7 us per unit (hand-out, Q/K fill, two-pass
     // first tile, epilogue) + ~0.95 us per (q-head tile, KV tile) pair.  Decode: ~2 us per item and stream plus its
@@ -327,7 +413,8 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     if (n_units > 0 && total_blocks > 0) {
         const int KT = D == 128 ? 128 : 64;
         double t_pre = 0.0;   // CTA-microseconds
-        for (const PreTile& t : tile_vec) {
+        for (int32_t i = 0; i < n_tiles; ++i) {
+            const PreTile& t = tiles[i];
             const double n_kv = std::ceil((double)(t.ctx + t.q_begin + t.q_rows) / KT);
             t_pre += (double)Hkv * (head_groups * 7.0 + n_kv * G * 0.95);
         }
@@ -342,15 +429,15 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
         } else {
             pre_ctas = (int32_t)std::lround(sms * t_pre / (t_pre + t_lat));
         }
-        pre_ctas = env_int("PA_PREFILL_CTAS", pre_ctas);
+        if (c.tune_prefill_ctas > 0) pre_ctas = c.tune_prefill_ctas;
         pre_ctas = std::max(1, std::min({pre_ctas, sms - 1, n_units}));
     } else if (n_units > 0) {
         pre_ctas = std::min(sms, n_units);
     }
     // ---- decode bundles
-    DecItem* items = reinterpret_cast<DecItem*>(ctx->h_stage);
-    int32_t n_items = 0, n_bundles = 0, n_split = 0;
-    std::vector<int32_t> bundle_start;
+    const int64_t off_b = align_up((int64_t)n_tiles * sizeof(PreTile), 256);
+    BundleCutter bc{reinterpret_cast<DecBundle*>(h_stage + off_b), ctx->max_bundles, ctx->max_split, 1};
+    int k = 0;
     if (total_blocks > 0) {
         // workers that start in the decode role; in a mixed launch the prefill CTAs join through the queue when
         // their units run out, so bundles are made finer (>= 2 per worker) and the tail balances dynamically
@@ -361,91 +448,70 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
         // roofline with 1 bundle per worker and 0.57 with 4); from ~16 GB on a launch lasts milliseconds and a second,
         // queue-drawn bundle per worker evens out unequal stream rates (C5: -5 %).  Mixed launches: 2 per worker.
         const double kv_bytes = (double)total_blocks * kBlock * D * 2 * 2;
-        int k = (mixed || kv_bytes >= 16e9) ? 2 : 1;
-        k = std::max(1, std::min(4, env_int("PA_BUNDLE_K", k)));
-        const int64_t min_blocks = std::max(1, env_int("PA_MIN_BUNDLE_BLOCKS", 2));
+        k = (mixed || kv_bytes >= 16e9) ? 2 : 1;
+        if (c.tune_bundles_per_stream > 0) k = c.tune_bundles_per_stream;
+        const int64_t min_blocks = c.tune_min_bundle_blocks > 0 ? c.tune_min_bundle_blocks : 2;
         const int64_t target = std::max(min_blocks, (total_blocks + W * k - 1) / (W * k));
-        bundle_start.reserve((size_t)(total_blocks / target + 2));
-        int64_t cur = 0;
-        bundle_start.push_back(0);
-        for (int s = 0; s < n_dec; ++s) {
-            const int32_t kv_len = h_ctx[s] + 1;
-            const int32_t nblk = (kv_len + kBlock - 1) / kBlock;
-            for (int g = 0; g < Hkv; ++g) {
-                int32_t pos = 0, first_item = n_items;
-                if ((nblk <= 16 || (int64_t)nblk * 4 <= target) && cur + nblk > target) {
+        bc.target = target;
+        for (int s = 0; s < n_dec && !bc.overflow; ++s) {
+            const int32_t nblk = (h_ctx[s] + kBlock) / kBlock;          // ceil((ctx + 1) / 16)
+            const int32_t grp0 = s * Hkv;
+            if (bc.cur + (int64_t)Hkv * nblk < target) {
+                // every group of the sequence joins the open bundle whole and no boundary is reached
+                bc.add_whole_sequence(grp0, Hkv, nblk);
+                continue;
+            }
+            const bool is_short = nblk <= 16 || (int64_t)nblk * 4 <= target;
+            for (int g = 0; g < Hkv && !bc.overflow; ++g) {
+                const int32_t grp = grp0 + g;
+                if (is_short && bc.cur + nblk > target) {
                     // a short group (<= 256 keys, or a quarter bundle) is never cut: partials + merge would cost
                     // more than the imbalance it leaves (a microsecond or two of streaming); it goes whole into this
                     // bundle or the next, whichever ends nearer the target
-                    if (cur + nblk - target > target - cur) {
-                        bundle_start.push_back(n_items);
-                        cur = 0;
-                    }
-                    if (n_items >= ctx->max_items) return fail(ctx, PA_ERR_INVALID, "pa_plan: decode item list overflow");
-                    items[n_items++] = DecItem{s, g, 0, nblk, kv_len, -1, 0, 1};
-                    cur += nblk;
-                    if (cur >= target) {
-                        bundle_start.push_back(n_items);
-                        cur = 0;
-                    }
+                    if (bc.cur + nblk - target > target - bc.cur) bc.close();
+                    bc.add(grp, 0, nblk, nblk);
+                    if (bc.cur >= target) bc.close();
                     continue;
                 }
-                while (pos < nblk) {
-                    const int32_t take = (int32_t)std::min<int64_t>(nblk - pos, target - cur);
-                    if (n_items >= ctx->max_items) return fail(ctx, PA_ERR_INVALID, "pa_plan: decode item list overflow");
-                    items[n_items++] = DecItem{s, g, pos, pos + take, kv_len, -1, 0, 1};
+                int32_t pos = 0, parts = 0;
+                const int32_t first_bundle = bc.n_bundles;
+                while (pos < nblk && !bc.overflow) {
+                    const int32_t take = (int32_t)std::min<int64_t>(nblk - pos, target - bc.cur);
+                    bc.add(grp, pos, pos + take, nblk);
                     pos += take;
-                    cur += take;
-                    if (cur == target) {
-                        bundle_start.push_back(n_items);
-                        cur = 0;
-                    }
+                    ++parts;
+                    if (bc.cur == target) bc.close();
                 }
-                const int32_t parts = n_items - first_item;
-                if (parts > 1) {
-                    if (n_split + parts > ctx->max_split) return fail(ctx, PA_ERR_INVALID, "pa_plan: partial slots overflow");
-                    for (int32_t i = 0; i < parts; ++i) {
-                        items[first_item + i].part_base = n_split;
-                        items[first_item + i].part_idx = i;
-                        items[first_item + i].n_parts = parts;
-                    }
-                    n_split += parts;
-                }
+                if (parts > 1) bc.mark_split(grp, first_bundle, parts);
             }
         }
-        if (bundle_start.back() != n_items) bundle_start.push_back(n_items);
-        n_bundles = (int32_t)bundle_start.size() - 1;
-        if (n_bundles > ctx->max_bundles) return fail(ctx, PA_ERR_INVALID, "pa_plan: bundle list overflow");
+        bc.close();
+        if (bc.overflow) return fail(ctx, PA_ERR_INVALID, "pa_plan: decode bundle / partial-slot list overflow");
     }
-    // ---- staging layout: items | bundle_start | tiles
-    int64_t off_b = align_up((int64_t)n_items * sizeof(DecItem), 256);
-    int32_t* h_bundles = reinterpret_cast<int32_t*>(ctx->h_stage + off_b);
-    for (int32_t i = 0; i <= n_bundles && n_bundles > 0; ++i) h_bundles[i] = bundle_start[i];
-    int64_t off_t = off_b + align_up((int64_t)(n_bundles + 1) * 4, 256);
-    if (n_tiles > 0) std::memcpy(ctx->h_stage + off_t, tile_vec.data(), (size_t)n_tiles * sizeof(PreTile));
-    const int64_t used = off_t + align_up((int64_t)n_tiles * sizeof(PreTile), 256);
+    const int32_t n_bundles = bc.n_bundles;
+    const int64_t used = off_b + align_up((int64_t)n_bundles * sizeof(DecBundle), 256);
 
     // ---- upload
     uint8_t* ws = static_cast<uint8_t*>(d_workspace);
     cudaError_t e = cudaMemsetAsync(ws + ctx->off_counters, 0, (size_t)(ctx->off_plan - ctx->off_counters), stream);
     if (e == cudaSuccess && used > 0)
-        e = cudaMemcpyAsync(ws + ctx->off_plan, ctx->h_stage, (size_t)used, cudaMemcpyHostToDevice, stream);
-    if (e == cudaSuccess) e = cudaEventRecord(ctx->stage_ev, stream);
+        e = cudaMemcpyAsync(ws + ctx->off_plan, h_stage, (size_t)used, cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->stage_ev[stage], stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "pa_plan(upload)");
-    ctx->stage_pending = true;
+    ctx->stage_pending[stage] = true;
+    ctx->stage_next = (stage + 1) % pa_ctx::kStages;
 
     PlanView& v = ctx->view;
     v.queue = reinterpret_cast<int32_t*>(ws + ctx->off_counters);
     v.group_counters = v.queue + 16;
-    v.items = reinterpret_cast<const DecItem*>(ws + ctx->off_plan);
-    v.bundle_start = reinterpret_cast<const int32_t*>(ws + ctx->off_plan + off_b);
-    v.tiles = reinterpret_cast<const PreTile*>(ws + ctx->off_plan + off_t);
+    v.tiles = reinterpret_cast<const PreTile*>(ws + ctx->off_plan);
+    v.bundles = reinterpret_cast<const DecBundle*>(ws + ctx->off_plan + off_b);
+    v.redo = reinterpret_cast<int2*>(ws + ctx->off_redo);
     v.part_ml = reinterpret_cast<float2*>(ws + ctx->off_part_ml);
     v.part_o = reinterpret_cast<float*>(ws + ctx->off_part_o);
-    v.n_items = n_items;
     v.n_bundles = n_bundles;
     v.n_tiles = n_tiles;
-    v.n_split = n_split;
+    v.n_split = bc.n_split;
     v.n_units = n_units;
     v.head_groups = head_groups;
     int32_t dec_ctas = 0;
@@ -453,10 +519,14 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     ctx->decode_ctas = dec_ctas;
     ctx->prefill_ctas = pre_ctas;
     ctx->p_in_tmem = prefill_mode == 0;
+    ctx->prefill_mode = prefill_mode;
+    ctx->bundles_per_stream = k;
+    ctx->n_items = bc.n_items;
     ctx->n_simple_tiles = prefill_mode == 2 ? n_tiles : 0;
     ctx->planned_n_tok = n_tok;
     ctx->launches_per_call = (dec_ctas + pre_ctas > 0) + (ctx->n_simple_tiles > 0);
     ctx->planned = true;
+    ctx->plan_host_ns = std::chrono::duration_cast<std::chrono::nanoseconds>(std::chrono::steady_clock::now() - t_begin).count();
     return PA_OK;
 }
 
@@ -469,6 +539,7 @@ int32_t pa_batch_attention(pa_ctx* ctx, const void* q, const void* k_pool, const
         return fail(ctx, PA_ERR_INVALID, "pa_batch_attention: null pointer");
     if (!(softmax_scale > 0.f) || !std::isfinite(softmax_scale))
         return fail(ctx, PA_ERR_INVALID, "pa_batch_attention: softmax_scale must be positive and finite");
+    if (int32_t rc = check_device(ctx, "pa_batch_attention")) return rc;
     if (ctx->tm_k_ptr != k_pool) {
         int32_t rc = make_pool_map(ctx, k_pool, &ctx->tmK);
         for (int i = 0; i < 5 && rc == PA_OK; ++i) rc = make_pool_map5(ctx, k_pool, &ctx->tails.k[i], 16 >> i, i == 0 ? 2 : 1);
@@ -516,13 +587,16 @@ int32_t pa_batch_attention(pa_ctx* ctx, const void* q, const void* k_pool, const
 int64_t pa_plan_info(const pa_ctx* ctx, int32_t which) {
     if (!ctx || !ctx->planned) return PA_ERR_INVALID;
     switch (which) {
-        case 0: return ctx->view.n_items;
+        case 0: return ctx->n_items;
         case 1: return ctx->view.n_bundles;
         case 2: return ctx->view.n_split;
         case 3: return ctx->view.n_tiles;
         case 4: return ctx->decode_ctas + ctx->prefill_ctas;
         case 5: return ctx->launches_per_call;
         case 6: return ctx->prefill_ctas;
+        case 7: return ctx->bundles_per_stream;
+        case 8: return ctx->prefill_mode;
+        case 9: return ctx->plan_host_ns;
         default: return PA_ERR_INVALID;
     }
 }
@@ -622,6 +696,41 @@ int32_t pa_timer_kappa(pa_ctx* ctx, int32_t n_tok, double* c, double* kappa, int
     const double k1 = c[0] + c[1] + c[2];
     if (k1 == 0.0) return fail(ctx, PA_ERR_TIMER, "pa_timer_kappa: K(1) == 0");
     *kappa = 2.0 * c[2] / k1;
+    return PA_OK;
+}
+
+// N3: Eq. 3 (base threshold under CFR) and Eq. 7 (crossover condition) — PAPER.md:L117-127, L184-191
+int32_t pa_crossover_theta0(double x, double* theta0, double* zeta) {
+    if (!theta0 || !zeta || !(x > 0.0) || !std::isfinite(x)) return PA_ERR_INVALID;
+    // f(t) = t/(1-t) + ln(1-t) - x is increasing on (0,1) from -x to +inf: Newton from above is monotone
+    // (f is convex), safeguarded by the bracket; f'(t) = t/(1-t)^2
+    double lo = 0.0, hi = 1.0, t = x < 0.5 ? std::min(0.999, std::sqrt(2.0 * x) + x) : 1.0 - 1.0 / (x + 2.0);
+    for (int it = 0; it < 200; ++it) {
+        const double f = t / (1.0 - t) + std::log1p(-t) - x;
+        if (f < 0.0) lo = t; else hi = t;
+        double tn = t - f * (1.0 - t) * (1.0 - t) / t;
+        if (!(tn > lo && tn < hi)) tn = 0.5 * (lo + hi);
+        if (std::fabs(tn - t) <= 1e-16 * t) { t = tn; break; }
+        t = tn;
+    }
+    *theta0 = t;
+    *zeta = -std::log1p(-t);
+    return PA_OK;
+}
+
+int32_t pa_crossover_eq7(const double* in, double* out) {
+    if (!in || !out) return PA_ERR_INVALID;
+    const double ap = in[0], bp = in[1], ad = in[2], bd = in[3], amb = in[4], bmb = in[5], muL = in[6], muO = in[7],
+                 zeta = in[8], k0 = in[9], N = in[10];
+    const double tok = muL + muO;
+    if (!(tok > 0.0) || !(k0 > 0.0) || !(N > 0.0)) return PA_ERR_INVALID;
+    const double beta_w = (bp * muL + bd * muO) / tok;
+    const double fixed_eb = (ap + ad * zeta * muO) / k0, fixed_mb = amb * (1.0 + muO) / N;
+    out[0] = bmb - beta_w;
+    out[1] = (fixed_eb - fixed_mb) / tok;
+    out[2] = beta_w;
+    out[3] = 1.0 / (fixed_eb + beta_w * tok);
+    out[4] = 1.0 / (fixed_mb + bmb * tok);
     return PA_OK;
 }
 

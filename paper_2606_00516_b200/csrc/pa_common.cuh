@@ -62,14 +62,6 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* m, 
         ::"r"(dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
         : "memory");
 }
-__device__ __forceinline__ void tma_load_4d_hint(uint32_t dst, const CUtensorMap* m, uint32_t bar, int c0, int c1,
-                                                 int c2, int c3, uint64_t policy) {
-    asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
-        "[%0], [%1, {%3, %4, %5, %6}], [%2], %7;"
-        ::"r"(dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(policy)
-        : "memory");
-}
 __device__ __forceinline__ void tma_load_5d_hint(uint32_t dst, const CUtensorMap* m, uint32_t bar, int c0, int c1,
                                                  int c2, int c3, int c4, uint64_t policy) {
     asm volatile(
@@ -93,11 +85,6 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* m, 
 __device__ __forceinline__ uint64_t policy_evict_first() {
     uint64_t p;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-__device__ __forceinline__ uint64_t policy_evict_last() {
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
 
@@ -155,38 +142,6 @@ __device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
     return d;
 }
-__device__ __forceinline__ uint64_t fadd2_rm(uint64_t a, uint64_t b) {     // round toward -inf
-    uint64_t d;
-    asm("add.rm.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ uint64_t fsub2(uint64_t a, uint64_t b) {
-    uint64_t d;
-    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-// 2^x for a pair, x in [-127, 127], on the FMA pipe instead of the 16-lane MUFU: floor by a round-down magic add,
-// degree-3 minimax polynomial of 2^f on [0,1) (max relative error 8.6e-5, below the bf16 rounding of P), exponent
-// inserted with an integer add.  Optional path of the prefill softmax (see kPolyMask in pa_prefill.cuh: off by
-// default, because the softmax groups turned out issue-bound, not MUFU-bound, on B200).
-__device__ __forceinline__ void exp2_poly2(uint64_t x, float& p0, float& p1) {
-    const uint64_t xr = fadd2_rm(x, pack_f2(12582912.f, 12582912.f));        // 1.5·2^23 + floor(x)
-    const uint64_t fl = fadd2(xr, pack_f2(-12582912.f, -12582912.f));         // floor(x), exact
-    const uint64_t f = fsub2(x, fl);                                          // x - floor(x) in [0, 1)
-    uint64_t p = ffma2(f, pack_f2(0.0770670548081398f, 0.0770670548081398f), pack_f2(0.22764497995376587f, 0.22764497995376587f));
-    p = ffma2(p, f, pack_f2(0.6951168179512024f, 0.6951168179512024f));
-    p = ffma2(p, f, pack_f2(1.f, 1.f));
-    float q0, q1, r0, r1;
-    unpack_f2(p, q0, q1);
-    unpack_f2(xr, r0, r1);
-    p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(r0) << 23));
-    p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(r1) << 23));
-}
-__device__ __forceinline__ float fast_rcp(float x) {
-    float y;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
 
 // ---------------------------------------------------------------- tcgen05 / TMEM (prefill path)
 __device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {   // one full warp
@@ -234,20 +189,8 @@ __device__ __forceinline__ uint32_t elect_one() {
         : "+r"(pred));
     return pred;
 }
-__device__ __forceinline__ void umma_ss_p(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
-    if (elect_one()) umma_ss(tmem_d, desc_a, desc_b, idesc, accumulate);
-}
-__device__ __forceinline__ void umma_ts_p(uint32_t tmem_d, uint32_t tmem_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
-    if (elect_one()) umma_ts(tmem_d, tmem_a, desc_b, idesc, accumulate);
-}
 __device__ __forceinline__ void umma_commit_p(uint32_t bar) {
     if (elect_one()) umma_commit(bar);
-}
-__device__ __forceinline__ void tma_load_4d_p(uint32_t dst, const CUtensorMap* m, uint32_t bar, int c0, int c1, int c2, int c3) {
-    if (elect_one()) tma_load_4d(dst, m, bar, c0, c1, c2, c3);
-}
-__device__ __forceinline__ void mbar_expect_tx_p(uint32_t bar, uint32_t bytes) {
-    if (elect_one()) mbar_expect_tx(bar, bytes);
 }
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
     asm volatile(
@@ -257,9 +200,6 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16
           "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
           "r"(taddr)
         : "memory");
-}
-__device__ __forceinline__ void mbar_inval(uint32_t bar) {
-    asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
 }
 // shared-memory matrix descriptor, 128-byte swizzle (layout type 2), descriptor version 1 (sm_100)
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
@@ -297,8 +237,6 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32
 }
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
-template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
 // 128-byte-swizzled tile addressing (TMA SWIZZLE_128B, tile base 1024-byte aligned):
 // element (row, col) of a [rows][64]-bf16 sub-tile whose rows are 128 B: 16-byte chunk index XOR (row & 7).

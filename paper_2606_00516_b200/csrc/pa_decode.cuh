@@ -4,9 +4,10 @@
 // private ring of 4 KB shared-memory slots plus a 2-entry item fifo, filled by a producer lane and
 // drained by one consumer warp; streams never synchronise with each other, only producer <-> consumer
 // through mbarriers, so HBM requests of a stream keep flowing across item and bundle boundaries.
-//   producer (warps 0-3, two lanes each, one stream per lane): walks the planner's bundles of
-//     (decode sequence, KV head, block range) items; per item it copies the item descriptor into the
-//     fifo and fetches the G query rows of that KV head with one TMA box per 64 columns; per block it
+//   producer (warps 0-3, two lanes each, one stream per lane): walks the planner's bundles — runs of the
+//     block stream of all (decode sequence, KV head) groups — and derives the (sequence, KV head, block
+//     range) items from the bundle descriptor and context_lens; per item it writes the item descriptor
+//     into the fifo and fetches the G query rows of that KV head with one TMA box per 64 columns; per block it
 //     looks up the block table and issues TMA tensor loads (cp.async.bulk.tensor, 128B swizzle) of the
 //     16-token K tile and V tile.  All of this runs ahead of the math by the ring depth, so block-table
 //     and descriptor latencies are off the consumers' critical path;
@@ -29,6 +30,8 @@ namespace pa {
 struct AttnParams {
     const __nv_bfloat16* q;       // [n_tok, Hq, D]
     __nv_bfloat16* out;           // [n_tok, Hq, D]
+    const __nv_bfloat16* k_pool;  // pools as plain pointers: the plain row loop (debug kernel, overflow redo) reads them
+    const __nv_bfloat16* v_pool;  //   directly; the decode and prefill roles see them through tensor maps only
     const int32_t* cu_seqlens_q;  // dev [n_seq+1]
     const int32_t* context_lens;  // dev [n_seq]
     const int32_t* block_tables;  // dev [n_seq, max_blocks_per_seq]
@@ -84,43 +87,68 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
     const uint64_t pol = policy_evict_first();
 
     uint32_t u_iss = 0, i_iss = 0;
-    int next_bundle = first_bundle;
-    if (next_bundle < 0) next_bundle = p.decode_workers + atomicAdd(&pl.queue[0], 1);
-    int item = 0, item_end = 0;
-    auto next_item = [&]() -> int {    // index of the stream's next item, -1 when the bundles are exhausted
-        while (item >= item_end) {
-            if (next_bundle >= pl.n_bundles) return -1;
-            item = __ldg(pl.bundle_start + next_bundle);
-            item_end = __ldg(pl.bundle_start + next_bundle + 1);
-            next_bundle = p.decode_workers + atomicAdd(&pl.queue[0], 1);   // result is needed one bundle later
+    // ---- bundle walk.  The stream's first bundle is static (or queue-drawn for a late joiner); every further one
+    // comes from the queue.  The queue index is requested two bundles ahead and the 32-byte descriptor one bundle
+    // ahead of their use, so neither the atomic nor the descriptor load is waited on where it is issued.
+    const int4* bundles = reinterpret_cast<const int4*>(pl.bundles);
+    int b_next = first_bundle;
+    if (b_next < 0) b_next = p.decode_workers + atomicAdd(&pl.queue[0], 1);
+    int4 nd0 = make_int4(0, 0, -1, 0), nd1 = nd0;        // descriptor of bundle b_next
+    bool have_next = b_next < pl.n_bundles;
+    if (have_next) { nd0 = __ldg(bundles + 2 * b_next); nd1 = __ldg(bundles + 2 * b_next + 1); }
+    int b_after = have_next ? p.decode_workers + atomicAdd(&pl.queue[0], 1) : pl.n_bundles;
+    int4 d0 = make_int4(0, 0, -1, 0), d1 = d0;           // current bundle: {grp_begin, blk_begin, grp_end, blk_end}, parts
+    int grp = 0, grp_last = -1;
+    // A group of the walk, with its context length in flight: {seq, kv head, blk_begin, blk_end or -1}, {ctx, part_base, part}
+    auto next_group = [&](int4& ga, int4& gb) -> bool {
+        if (grp > grp_last) {
+            if (!have_next) return false;
+            d0 = nd0; d1 = nd1;
+            grp = d0.x; grp_last = d0.z;
+            have_next = b_after < pl.n_bundles;
+            if (have_next) {
+                nd0 = __ldg(bundles + 2 * b_after); nd1 = __ldg(bundles + 2 * b_after + 1);
+                b_after = p.decode_workers + atomicAdd(&pl.queue[0], 1);
+            }
         }
-        return item++;
+        const int seq = grp / p.Hkv, kvh = grp - seq * p.Hkv;
+        const bool first = grp == d0.x, last = grp == d0.z;
+        ga = make_int4(seq, kvh, first ? d0.y : 0, last ? d0.w : -1);
+        gb = make_int4(__ldg(p.context_lens + seq), first ? d1.x : (last ? d1.z : -1), first ? d1.y : (last ? d1.w : 1), 0);
+        ++grp;
+        return true;
+    };
+    // turns a fetched group into the item descriptor (DecItem layout) once its context length has arrived
+    auto resolve = [&](int4& ga, int4& gb) {
+        const int kv_len = gb.x + 1, nblk = (kv_len + kBlock - 1) / kBlock;
+        if (ga.w < 0) ga.w = nblk;
+        const int part = gb.z;
+        gb = make_int4(kv_len, gb.y, gb.y < 0 ? 0 : (part >> 16), gb.y < 0 ? 1 : (part & 0xffff));
     };
     // Two-deep software pipeline over items so that no load is waited on where it is issued:
-    //   stage 2: descriptor of item i+2 in flight;  stage 1: descriptor of item i+1 arrived, its first block id in flight.
+    //   stage 2: context length of item i+2 in flight;  stage 1: item i+1 resolved, its first block ids in flight.
     int4 a1 = make_int4(0, 0, 0, 0), b1 = a1, a2 = a1, b2 = a1;
     int blkid1 = 0, blkid1n = 0;      // ids of the first two blocks of the stage-1 item
-    int i2 = next_item();
-    if (i2 >= 0) { a2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2)); b2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2) + 1); }
-    bool v1 = i2 >= 0;
-    a1 = a2; b1 = b2;
+    bool v2 = next_group(a2, b2);
+    bool v1 = v2;
     if (v1) {
+        a1 = a2; b1 = b2;
+        resolve(a1, b1);
         blkid1 = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z);
         if (a1.z + 1 < a1.w) blkid1n = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z + 1);
-        i2 = next_item();
-        if (i2 >= 0) { a2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2)); b2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2) + 1); }
+        v2 = next_group(a2, b2);
     }
     while (v1) {
         const int4 a = a1, b = b1;
         int blkid = blkid1, blkid_n = blkid1n;
         // ---- advance the pipeline
-        v1 = i2 >= 0;
+        v1 = v2;
         if (v1) {
             a1 = a2; b1 = b2;
+            resolve(a1, b1);
             blkid1 = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z);
             if (a1.z + 1 < a1.w) blkid1n = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z + 1);
-            i2 = next_item();
-            if (i2 >= 0) { a2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2)); b2 = __ldg(reinterpret_cast<const int4*>(pl.items + i2) + 1); }
+            v2 = next_group(a2, b2);
         }
         // ---- open the item: descriptor + Q rows into the fifo entry
         const int seq = a.x, kvh = a.y, blk_end = a.w, kv_len = b.x;

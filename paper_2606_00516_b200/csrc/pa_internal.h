@@ -9,10 +9,10 @@ constexpr int kBlock = 16;          // KV block size b (tokens)
 constexpr int kDecodeWarps = 8;     // persistent decode workers (warps) per CTA
 constexpr int kMaxGroup = 8;        // max q heads per KV head (N of the decode MMA)
 constexpr int kQTile = 128;         // prefill query-tile rows
-constexpr int kKvTile = 128;        // prefill KV-tile keys
 
 // One decode work item: a run of whole KV blocks of one (decode sequence, KV head).
-// "(seq, kv head, kv chunk)".
+// "(seq, kv head, kv chunk)".  Items are not stored in HBM: the producer lane of a stream derives
+// them from its bundle descriptor (below) and context_lens, and hands them to the consumer warp through shared memory.
 struct DecItem {
     int32_t seq;        // sequence index in the batch
     int32_t kv_head;    // KV head g
@@ -24,6 +24,19 @@ struct DecItem {
     int32_t n_parts;    // parts of the group (1 = write the output row directly)
 };
 static_assert(sizeof(DecItem) == 32, "DecItem layout");
+
+// One decode bundle: a contiguous run of the block stream formed by all (decode sequence, KV head) groups in
+// group order (group id = seq * Hkv + kv head).  It starts at block `blk_begin` of group `grp_begin` and ends with
+// block `blk_end - 1` of group `grp_end` (blk_end < 0: the group's last block); every group strictly between the two
+// is covered whole.  A group that a bundle boundary cuts is a split group: its parts write partials into slots
+// part_base + part_idx and the last-arriving part merges them.  Only the first and the last group of a bundle can be
+// split (part_base < 0: not split).  The planner writes O(bundles) of these instead of O(groups) items.
+struct DecBundle {
+    int32_t grp_begin, blk_begin, grp_end, blk_end;
+    int32_t first_part_base, first_part;   // first group: slot base, (part_idx << 16) | n_parts
+    int32_t last_part_base, last_part;     // last group (when grp_end > grp_begin): the same
+};
+static_assert(sizeof(DecBundle) == 32, "DecBundle layout");
 
 // One prefill tile: up to kQTile consecutive query rows of one prefill chunk (all heads handled by the kernel grid).
 struct PreTile {
@@ -39,10 +52,10 @@ static_assert(sizeof(PreTile) == 32, "PreTile layout");
 
 // Device-side view of the planned workspace (all pointers into the caller's workspace buffer).
 struct PlanView {
-    int32_t* queue;            // [0] next decode bundle, [1] exited CTAs, [2] next prefill unit (all self-resetting)
+    int32_t* queue;            // [0] next decode bundle, [1] exited CTAs, [2] next prefill unit, [3] rows to redo (all self-resetting)
     int32_t* group_counters;   // [num_decode_seqs * Hkv] arrivals of split groups (self-resetting)
-    const DecItem* items;      // decode items in bundle order
-    const int32_t* bundle_start; // [n_bundles + 1] item index ranges
+    const DecBundle* bundles;  // [n_bundles] decode bundles
+    int2* redo;                // prefill rows whose one-pass softmax overflowed: {tile index, (row in tile << 8) | q head}
     const PreTile* tiles;      // prefill tiles
     float2* part_ml;           // [slots][kMaxGroup] (m in log2 domain, l)
     float* part_o;             // [slots][G][D] unnormalised partial outputs

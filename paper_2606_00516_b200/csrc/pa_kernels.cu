@@ -175,11 +175,30 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
         }
         __syncthreads();
     }
+    // The last CTA to leave resets the queues for the next launch and recomputes, with the plain row loop, the prefill
+    // rows whose one-pass softmax overflowed (normally none).  Pattern: writers fence before the counting atomic,
+    // the last arriver fences after it.
+    int* last_flag = reinterpret_cast<int*>(&ctrl->unit[0]);
     if (threadIdx.x == 0) {
-        if (atomicAdd(&pl.queue[1], 1) == (int)gridDim.x - 1) {
+        __threadfence();
+        *last_flag = atomicAdd(&pl.queue[1], 1) == (int)gridDim.x - 1;
+    }
+    __syncthreads();
+    if (*last_flag) {
+        __threadfence();
+        const int n_redo = *reinterpret_cast<volatile int*>(&pl.queue[3]);
+        for (int i = threadIdx.x >> 5; i < n_redo; i += kAttnThreads / 32) {
+            const int2 e = __ldcg(pl.redo + i);
+            const PreTile t = pl.tiles[e.x];
+            const int j = t.q_begin + (e.y >> 8);
+            simple_row<D>(p, t.seq, t.ctx, j, (int64_t)t.row0 + j, e.y & 0xff, lane_id());
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
             pl.queue[0] = 0;
             pl.queue[1] = 0;
             pl.queue[2] = 0;
+            pl.queue[3] = 0;
             __threadfence();
         }
     }
@@ -204,6 +223,8 @@ cudaError_t launch_attention(const AttnLaunch& a, cudaStream_t stream, int* laun
     AttnParams p;
     p.q = reinterpret_cast<const __nv_bfloat16*>(a.q);
     p.out = reinterpret_cast<__nv_bfloat16*>(a.out);
+    p.k_pool = reinterpret_cast<const __nv_bfloat16*>(a.k_pool);
+    p.v_pool = reinterpret_cast<const __nv_bfloat16*>(a.v_pool);
     p.cu_seqlens_q = a.cu_seqlens_q;
     p.context_lens = a.context_lens;
     p.block_tables = a.block_tables;
@@ -247,9 +268,9 @@ cudaError_t launch_attention(const AttnLaunch& a, cudaStream_t stream, int* laun
     if (a.n_simple_tiles > 0) {
         dim3 grid(a.n_simple_tiles, a.sh.Hq), block(128);
         if (a.sh.D == 128)
-            pa_simple_kernel<128><<<grid, block, 0, stream>>>(p, (const __nv_bfloat16*)a.k_pool, (const __nv_bfloat16*)a.v_pool);
+            pa_simple_kernel<128><<<grid, block, 0, stream>>>(p);
         else
-            pa_simple_kernel<256><<<grid, block, 0, stream>>>(p, (const __nv_bfloat16*)a.k_pool, (const __nv_bfloat16*)a.v_pool);
+            pa_simple_kernel<256><<<grid, block, 0, stream>>>(p);
         ++launches;
         e = cudaGetLastError();
     }

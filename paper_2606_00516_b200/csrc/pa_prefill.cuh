@@ -29,15 +29,6 @@
 namespace pa {
 
 constexpr int kAttnThreads = 384;   // 12 warps: control warpgroup + two softmax warpgroups
-// pairs (of the 16 pairs of a 32-column chunk) whose exponentials run on the FMA pipe (exp2_poly2) instead of MUFU.
-// Measured on B200 (C4 r=0, 1107 TFLOP/s with mask 0): 25 % of the pairs -> 990, 50 % -> 862 TFLOP/s.  The softmax
-// groups are bound by instruction issue, not by MUFU throughput, so the polynomial (5 extra instructions per
-// element) loses; the default sends every exponential to MUFU.  -DPA_POLY_MASK=0x.... re-enables it.
-#ifndef PA_POLY_MASK
-#define PA_POLY_MASK 0x0000u
-#endif
-constexpr uint32_t kPolyMask = PA_POLY_MASK;
-
 template <int D, bool kPinTmem>
 struct PrefillCfg {
     static constexpr int NQ = (D == 128) ? 2 : 1;              // q-head tiles per unit
@@ -354,12 +345,8 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                             const uint64_t x = ffma2(pack_f2(s0, s1), sl2, neg2);
                             float x0, x1, p0, p1;
                             unpack_f2(x, x0, x1);
-                            if ((kPolyMask >> (i >> 1)) & 1u) {
-                                exp2_poly2(pack_f2(fmaxf(x0, -127.f), fmaxf(x1, -127.f)), p0, p1);
-                            } else {
-                                p0 = fast_exp2(x0);
-                                p1 = fast_exp2(x1);
-                            }
+                            p0 = fast_exp2(x0);
+                            p1 = fast_exp2(x1);
                             lsum = fadd2(lsum, pack_f2(p0, p1));
                             pk[i >> 1] = pack_bf16x2(p0, p1);
                         }
@@ -426,7 +413,14 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                 oph ^= 1u;
                 tc_fence_after();
                 const float inv = 1.f / l;
-                const bool valid = row < tile.q_rows;
+                bool valid = row < tile.q_rows;
+                if (valid && !(l <= 3.0e38f)) {
+                    // the one-pass softmax overflowed (a tile outgrew everything before it by > 2^127): hand the row
+                    // to the plain loop that the last CTA of the launch runs (include/pa.h, "Range")
+                    pl.redo[atomicAdd(&pl.queue[3], 1)] = make_int2(ti, (row << 8) | (h_first + t));
+                    __threadfence();
+                    valid = false;
+                }
                 uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)(tile.row0 + tile.q_begin + row) * p.Hq + h_first + t) * D);
 #pragma unroll
                 for (int c = 0; c < D / 32; ++c) {

@@ -28,6 +28,8 @@ def _load():
         _lib = C.CDLL(_LIB_PATH)
         _lib.synth_fill_bf16.argtypes = [C.c_void_p, C.c_int64, C.c_uint64, C.c_uint32, C.c_int64, C.c_void_p]
         _lib.synth_fill_bf16.restype = C.c_int32
+        _lib.synth_read_probe.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
+        _lib.synth_read_probe.restype = C.c_int32
     return _lib
 
 
@@ -38,6 +40,16 @@ def fill_bf16(t: torch.Tensor, seed: int, tensor_id: int, start: int = 0) -> tor
     if rc != 0:
         raise RuntimeError(f"synth_fill_bf16 failed: cuda error {rc}")
     return t
+
+
+def read_probe(buf: torch.Tensor, mode: int, sink: torch.Tensor) -> None:
+    """Enqueue one read-only pass over ``buf`` on the current stream (mode 0: ld.global, 1: bulk copies into shared
+    memory).  Measurement support for bench.py's read ceiling; ``sink`` is a 1-element int64 CUDA tensor."""
+    nbytes = buf.numel() * buf.element_size()
+    rc = _load().synth_read_probe(buf.data_ptr(), nbytes - nbytes % 16384, mode, sink.data_ptr(),
+                                  torch.cuda.current_stream().cuda_stream)
+    if rc != 0:
+        raise RuntimeError(f"synth_read_probe failed: cuda error {rc}")
 
 
 @dataclass
@@ -54,9 +66,11 @@ class DeviceBatch:
     out: torch.Tensor
 
 
-def materialise(batch: Batch, device="cuda:0", pools=None) -> DeviceBatch:
+def materialise(batch: Batch, device="cuda:0", pools=None, refill: bool = True) -> DeviceBatch:
     """Allocate and fill every tensor of the batch on the device.  ``pools`` lets callers reuse one
-    (k_pool, v_pool) pair across batches of the same shape/num_blocks (it is refilled)."""
+    (k_pool, v_pool) pair across batches of the same shape/num_blocks; it is refilled with the batch's own streams
+    unless ``refill`` is False (timing loops that share one resident pool between batches: the values stay seeded
+    N(0,1) bf16, only the seed is another batch's)."""
     sh = batch.shape
     dev = torch.device(device)
     n = batch.n_tok
@@ -75,8 +89,9 @@ def materialise(batch: Batch, device="cuda:0", pools=None) -> DeviceBatch:
             fill_bf16(q, batch.seed, gen.TENSOR_Q)
             fill_bf16(k_new, batch.seed, gen.TENSOR_K_NEW)
             fill_bf16(v_new, batch.seed, gen.TENSOR_V_NEW)
-        fill_bf16(k_pool, batch.seed, gen.TENSOR_K_POOL)
-        fill_bf16(v_pool, batch.seed, gen.TENSOR_V_POOL)
+        if refill or pools is None:
+            fill_bf16(k_pool, batch.seed, gen.TENSOR_K_POOL)
+            fill_bf16(v_pool, batch.seed, gen.TENSOR_V_POOL)
     out = torch.zeros_like(q)
     return DeviceBatch(batch, q, k_new, v_new, k_pool, v_pool,
                        torch.from_numpy(batch.cu_seqlens_q).to(dev), torch.from_numpy(batch.context_lens).to(dev),

@@ -56,3 +56,87 @@ extern "C" int32_t synth_fill_bf16(void* dst, int64_t n, uint64_t seed, uint32_t
     fill_kernel<<<grid, block, 0, static_cast<cudaStream_t>(stream)>>>(static_cast<uint16_t*>(dst), n, key, start);
     return (int32_t)cudaGetLastError();
 }
+
+// ------------------------------------------------------------------------------------------------
+// Read-only HBM streaming probes (bench.py "peaks.read_probe_gbs"; SURVEY §7 "HBM target denominator").
+// The decode path is read-dominated, and a copy (read + write) understates what a read stream can reach,
+// so bench.py measures the read ceiling in the same run with two plain probes and takes the faster one:
+//   mode 0: every thread sums 16-byte ld.global.nc loads, 8 in flight per thread (grid-stride over 8-vector chunks);
+//   mode 1: one thread per CTA streams 16 KB bulk copies (cp.async.bulk global -> shared, mbarrier complete_tx)
+//           through a shared-memory ring — the access pattern of TMA-fed kernels; the data is not consumed.
+// Measurement support only: no arithmetic of the method.
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+__global__ void __launch_bounds__(512) read_probe_ldg(const uint4* __restrict__ src, int64_t n_vec, unsigned long long* sink) {
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t nthreads = (int64_t)gridDim.x * blockDim.x;
+    uint32_t acc = 0;
+    int64_t i = tid;
+    for (; i + 7 * nthreads < n_vec; i += 8 * nthreads) {
+        uint4 v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+            asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+                         : "=r"(v[k].x), "=r"(v[k].y), "=r"(v[k].z), "=r"(v[k].w) : "l"(src + i + k * nthreads));
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc += v[k].x ^ v[k].y ^ v[k].z ^ v[k].w;
+    }
+    for (; i < n_vec; i += nthreads) { const uint4 v = __ldg(src + i); acc += v.x ^ v.y ^ v.z ^ v.w; }
+    if (acc == 0x9E3779B9u) atomicAdd(sink, 1ull);     // keeps the loads alive; practically never taken
+}
+
+constexpr int kBulkBytes = 16384, kBulkStages = 12;
+
+__global__ void __launch_bounds__(32) read_probe_bulk(const uint8_t* __restrict__ src, int64_t n_chunks, unsigned long long* sink) {
+    extern __shared__ __align__(128) uint8_t ring[];
+    __shared__ __align__(8) uint64_t full[kBulkStages];
+    if (threadIdx.x != 0) return;
+    for (int s = 0; s < kBulkStages; ++s)
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(&full[s])) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    const uint32_t ring_u32 = (uint32_t)__cvta_generic_to_shared(ring);
+    int64_t issued = 0, waited = 0, c = blockIdx.x;
+    for (;;) {
+        if (c < n_chunks && issued - waited < kBulkStages) {
+            const int s = (int)(issued % kBulkStages);
+            const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&full[s]);
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(kBulkBytes) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(ring_u32 + s * kBulkBytes), "l"(src + c * kBulkBytes), "r"(kBulkBytes), "r"(bar) : "memory");
+            ++issued;
+            c += gridDim.x;
+        } else if (waited < issued) {
+            const int s = (int)(waited % kBulkStages);
+            const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&full[s]), parity = (uint32_t)((waited / kBulkStages) & 1);
+            uint32_t ok = 0;
+            while (!ok)
+                asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                             : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+            ++waited;
+        } else {
+            break;
+        }
+    }
+    if (ring[0] == 0x5A && ring[1] == 0xA5 && ring[2] == 0x3C && ring[3] == 0xC3) atomicAdd(sink, 1ull);
+}
+
+}  // namespace
+
+// Reads `bytes` (multiple of 16 KB) from dev pointer `src` once on `stream`; `sink` = dev uint64 scratch.
+// mode 0: ld.global probe, mode 1: bulk-copy probe.  Returns the cudaError_t of the launch.
+extern "C" int32_t synth_read_probe(const void* src, int64_t bytes, int32_t mode, void* sink, void* stream) {
+    if (bytes <= 0 || bytes % kBulkBytes != 0) return (int32_t)cudaErrorInvalidValue;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (mode == 0) {
+        read_probe_ldg<<<sms * 4, 512, 0, st>>>(static_cast<const uint4*>(src), bytes / 16, static_cast<unsigned long long*>(sink));
+    } else {
+        const int smem = kBulkBytes * kBulkStages;
+        cudaFuncSetAttribute(read_probe_bulk, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        read_probe_bulk<<<sms, 32, smem, st>>>(static_cast<const uint8_t*>(src), bytes / kBulkBytes, static_cast<unsigned long long*>(sink));
+    }
+    return (int32_t)cudaGetLastError();
+}

@@ -192,9 +192,10 @@ def config3(n_seq: int = 256, lo: int = 512, hi: int = 4096, num_blocks: int = 6
     return make_batch("C3-gemma3-1b-decode", GEMMA3_1B, 3, [1] * n_seq, ctx, n_seq, num_blocks=num_blocks)
 
 
-def config4(r: float, n_tok: int = 8192, chunk: int = 2048) -> Batch:
+def config4(r: float, n_tok: int = 8192, chunk: int = 2048, num_blocks: int | None = None) -> Batch:
     """C4 Qwen3-8B shape: decode ctx lognormal(median 2048, σ 0.7 — R14) clipped [256, 8192];
-    prefill chunks of 2048 over prior ctx ~ U{0..4096}; seed 400+i; pool sized to the batch."""
+    prefill chunks of 2048 over prior ctx ~ U{0..4096}; seed 400+i; pool sized to the batch, or ``num_blocks``
+    (``c4_pool_blocks()``: the one pool that serves every r, as bench.py and the full-size parity tests use it)."""
     i = int(round(10 * r))
     nd = n_decode_for(r, n_tok)
     npre = n_tok - nd
@@ -204,7 +205,19 @@ def config4(r: float, n_tok: int = 8192, chunk: int = 2048) -> Batch:
     pc = rng.integers(0, 4097, nch + (1 if rem else 0))
     q = [1] * nd + [chunk] * nch + ([rem] if rem else [])
     c = list(dc) + list(pc)
-    return make_batch(f"C4-qwen3-8b-n{n_tok}-r{r:.1f}", QWEN3_8B, 400 + i, q, c, nd)
+    return make_batch(f"C4-qwen3-8b-n{n_tok}-r{r:.1f}", QWEN3_8B, 400 + i, q, c, nd, num_blocks=num_blocks)
+
+
+_C4_POOL_BLOCKS = None
+
+
+def c4_pool_blocks() -> int:
+    """Blocks of the one pool pair that holds any C4 batch (n_tok 8192, every r of the sweep): the largest need
+    (r = 1.0: ~1.3 M blocks x 32 KB per pool = ~42 GB per pool), rounded up to a multiple of 1024."""
+    global _C4_POOL_BLOCKS
+    if _C4_POOL_BLOCKS is None:
+        _C4_POOL_BLOCKS = max(config4(i / 10).num_blocks for i in range(11))
+    return _C4_POOL_BLOCKS
 
 
 def config5(variant: str = "r1.0", n_dec: int = 1024, num_blocks: int | None = None) -> Batch:

@@ -85,15 +85,53 @@ def test_kv_append_and_gather_bit_exact(name):
         assert (sdev.bits(k_out) == kg).all() and (sdev.bits(v_out) == vg).all()
 
 
-@pytest.mark.parametrize("mode", [0, 1])      # prefill variant: P staged in TMEM (default) / in shared memory
+MODE_FLAGS = {0: 0, 1: binding.PA_FLAG_PREFILL_P_SMEM}     # prefill variant: P staged in TMEM (default) / in shared memory
+
+
+@pytest.mark.parametrize("mode", [0, 1])
 @pytest.mark.parametrize("name", SMALL)
-def test_attention_parity_small(name, mode, monkeypatch):
-    monkeypatch.setenv("PA_PREFILL_MODE", str(mode))
+def test_attention_parity_small(name, mode):
     batch = _small_case(name)
     inp = helpers.host_inputs(batch)
-    d = gc.run_gpu(batch, inp)
-    ref, _, _ = gc.run_oracle(batch, inp)
+    d = gc.run_gpu(batch, inp, flags=MODE_FLAGS[mode])
+    assert d["pa"].plan_info(8) == mode
+    ref, kp, vp = gc.run_oracle(batch, inp)
+    assert (sdev.bits(d["k_pool"]) == kp).all() and (sdev.bits(d["v_pool"]) == vp).all()
     gc.check_close(sdev.bits(d["out"]), ref, f"{name}/mode{mode}")
+
+
+@pytest.mark.parametrize("order", ["plan_between", "graph"])
+@pytest.mark.parametrize("name", ["C1", "ragged-g4-d128", "ragged-g4-d256", "edge-lens", "decode-only", "prefill-only"])
+def test_call_orders_small(name, order):
+    """The same result whether the plan is uploaded between append and attention (round-1 test order) or the
+    append -> attention pair is replayed from a CUDA graph after planning (bench.py's headline loop)."""
+    batch = _small_case(name)
+    inp = helpers.host_inputs(batch)
+    d = gc.run_gpu(batch, inp, order=order, repeat=2)
+    ref, kp, vp = gc.run_oracle(batch, inp)
+    assert (sdev.bits(d["k_pool"]) == kp).all() and (sdev.bits(d["v_pool"]) == vp).all()
+    gc.check_close(sdev.bits(d["out"]), ref, f"{name}/{order}")
+
+
+@pytest.mark.parametrize("tune", [dict(tune_prefill_ctas=1), dict(tune_prefill_ctas=100), dict(tune_bundles_per_stream=4),
+                                  dict(tune_bundles_per_stream=1, tune_min_bundle_blocks=1),
+                                  dict(tune_min_bundle_blocks=64)])
+def test_planner_knobs_change_the_schedule_not_the_result(tune):
+    """pa_config.tune_* (the documented replacements of round 1's environment variables): any setting is a valid plan."""
+    batch = _small_case("ragged-g4-d128")
+    inp = helpers.host_inputs(batch)
+    ref, _, _ = gc.run_oracle(batch, inp)
+    d = gc.run_gpu(batch, inp, tune=tune)
+    if "tune_prefill_ctas" in tune:
+        assert d["pa"].plan_info(6) == min(tune["tune_prefill_ctas"], 147, d["pa"].plan_info(3) * 8 * 2)
+    if "tune_bundles_per_stream" in tune:
+        assert d["pa"].plan_info(7) == tune["tune_bundles_per_stream"]
+    gc.check_close(sdev.bits(d["out"]), ref, f"knobs/{tune}")
+    long = workloads.make_batch("split", workloads.GEMMA3_1B, 209, [1, 1, 1], [5000, 3333, 4097], 3)
+    inp = helpers.host_inputs(long)
+    ref, _, _ = gc.run_oracle(long, inp)
+    d = gc.run_gpu(long, inp, tune=tune, repeat=2)
+    gc.check_close(sdev.bits(d["out"]), ref, f"knobs-long/{tune}")
 
 
 @pytest.mark.parametrize("name", ["C1", "ragged-g4-d128", "ragged-g4-d256"])
@@ -118,11 +156,10 @@ def test_split_kv_groups_merge_in_launch():
 
 @pytest.mark.parametrize("mode", [0, 1])
 @pytest.mark.parametrize("shape_name", ["QWEN3_4B", "GEMMA3_1B"])
-def test_prefill_running_max_growth(shape_name, mode, monkeypatch):
+def test_prefill_running_max_growth(shape_name, mode):
     """Scores that grow along the keys: the prefill softmax exponentiates a tile against the reference max left by
     earlier tiles, so the three regimes must all match the oracle: growth below 2^8 (reference kept),
     above 2^8 (lazy rescale of l and O at the next tile) and above 2^64 within one tile (exact power-of-two fix-up)."""
-    monkeypatch.setenv("PA_PREFILL_MODE", str(mode))
     W = workloads
     shape = getattr(W, shape_name)
     ctx, q_len = 500, 300
@@ -141,9 +178,39 @@ def test_prefill_running_max_growth(shape_name, mode, monkeypatch):
             inp["k_pool"][int(batch.block_tables[1, t // b]), :, t % b, 0] = v
         else:
             inp["k_new"][row0 + t - ctx, :, 0] = v
-    d = gc.run_gpu(batch, inp)
+    d = gc.run_gpu(batch, inp, flags=MODE_FLAGS[mode])
     ref, _, _ = gc.run_oracle(batch, inp)
     gc.check_close(sdev.bits(d["out"]), ref, f"growth/{shape_name}/mode{mode}")
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("shape_name", ["QWEN3_4B", "GEMMA3_1B"])
+def test_prefill_overflow_rows_are_recomputed(shape_name, mode):
+    """Beyond the one-pass limit: the scores of one 128-key tile exceed everything before them by > 2^127 (here ~200
+    and ~400 nats).  The tensor-core pass overflows for those rows, the launch detects it (row sum not finite) and
+    its last CTA recomputes them with the plain loop (include/pa.h "Range"): the result is still the oracle's."""
+    W = workloads
+    shape = getattr(W, shape_name)
+    ctx, q_len = 500, 300
+    batch = W.make_batch("overflow", shape, 217, [1, q_len, 70], [40, ctx, 300], 1)
+    inp = helpers.host_inputs(batch)
+    scale = batch.softmax_scale
+    gain = {2: 200.0 / (8.0 * scale), 4: 400.0 / (8.0 * scale), 5: 0.0}     # nats above the N(0,1) background, per 128 keys
+    b = shape.block_size
+    bits = lambda v: gen.f32_to_bf16(np.array([v], dtype=np.float32))[0]
+    row0 = int(batch.cu_seqlens_q[1])
+    inp["q"][row0:row0 + q_len, :, 0] = bits(8.0)
+    for t in range(ctx + q_len):
+        if t // 128 not in gain:
+            continue
+        v = bits(gain[t // 128])
+        if t < ctx:
+            inp["k_pool"][int(batch.block_tables[1, t // b]), :, t % b, 0] = v
+        else:
+            inp["k_new"][row0 + t - ctx, :, 0] = v
+    d = gc.run_gpu(batch, inp, flags=MODE_FLAGS[mode], repeat=2)        # repeat: the redo counter must self-reset
+    ref, _, _ = gc.run_oracle(batch, inp)
+    gc.check_close(sdev.bits(d["out"]), ref, f"overflow/{shape_name}/mode{mode}")
 
 
 @pytest.mark.parametrize("shape_name,ctx", [("GEMMA3_1B", 150000), ("QWEN3_30B_A3B", 60000)])
@@ -157,6 +224,28 @@ def test_one_long_sequence_split_over_every_worker(shape_name, ctx):
     gc.check_sampled_sequences(batch, d, [0], what=f"long1/{shape_name}")
 
 
+@pytest.mark.parametrize("shape_name,ctx", [("GEMMA3_1B", 150000), ("QWEN3_30B_A3B", 60000)])
+def test_long_sequence_with_peaked_scores(shape_name, ctx):
+    """The same split-over-every-stream launch with O(1) outputs: four keys far apart score ~25 nats above the
+    N(0,1) background (which carries e^12..13 of mass in total), so the result is essentially the mean of their V
+    rows and an error in any part's (m, l, o) or in the merge shows at full scale, not at the 1/sqrt(kv_len) scale of
+    a flat softmax."""
+    W = workloads
+    shape = getattr(W, shape_name)
+    batch = W.make_batch("long1-peaked", shape, 218, [1], [ctx], 1)
+    peaks = [7, ctx // 3 + 5, (2 * ctx) // 3 + 11, ctx - 2]
+
+    def peak(d):
+        d["q"][0, :, 0] = 8.0
+        val = 25.0 / (8.0 * batch.softmax_scale)
+        for t in peaks:
+            d["k_pool"][int(batch.block_tables[0, t // 16]), :, t % 16, 0] = val
+    d = gc.run_gpu(batch, None, repeat=2, pre_append=peak)
+    assert d["pa"].plan_info(2) >= 148
+    gc.check_sampled_sequences(batch, d, [0], what=f"long1-peaked/{shape_name}")
+    assert float(d["out"].float().abs().mean()) > 0.1, "outputs should be O(1) in this case"
+
+
 def test_repeated_launches_are_deterministic_and_reset_state():
     batch = _small_case("ragged-g4-d128")
     inp = helpers.host_inputs(batch)
@@ -165,24 +254,29 @@ def test_repeated_launches_are_deterministic_and_reset_state():
     assert (sdev.bits(d1["out"]) == sdev.bits(d2["out"])).all()
 
 
-@pytest.mark.parametrize("r", [0.0, 0.1, 0.5, 1.0])
-def test_config2_parity(r):
+def _device_pool_is_the_host_stream(batch, pool_bits, tensor_id, seed=1):
+    """The device-filled pool must be the seeded host stream (sampled), so the oracle's inputs are not the CUDA path's."""
+    idx = np.random.default_rng(seed).integers(0, batch.pool_elems(), 4096)
+    valid = helpers.slot_valid_mask(batch, "ctx")
+    flat_valid = np.broadcast_to(valid[:, None, :, None], pool_bits.shape).reshape(-1)[idx]
+    host = gen.bf16_normal_at(batch.seed, tensor_id, idx.astype(np.uint64))
+    assert (pool_bits.reshape(-1)[idx][flat_valid] == host[flat_valid]).all()
+
+
+@pytest.mark.parametrize("order", ["plan_first", "graph"])
+@pytest.mark.parametrize("r", [i / 10 for i in range(11)])
+def test_config2_timed_sequence_all_rows(r, order):
+    """C2 at every r of the sweep, in exactly the sequence bench.py times: pa_plan first, then kv_append and
+    batch_attention back to back (the attention launch comes up under the append by programmatic dependent launch),
+    eagerly and replayed from a CUDA graph.  ALL 2048 x 32 output rows vs the oracle; both pools bit-exact."""
     batch = workloads.config2(r)
-    d = gc.run_gpu(batch, None)
+    d = gc.run_gpu(batch, None, order=order, repeat=2)
     inp = dict(q=batch.q_bits(), k_new=batch.kv_new_bits()[0], v_new=batch.kv_new_bits()[1],
                k_pool=sdev.bits(d["pool_before"][0]), v_pool=sdev.bits(d["pool_before"][1]))
-    # the device-filled pool must be the host stream (sampled), so the oracle's inputs are not the CUDA path's
-    idx = np.random.default_rng(1).integers(0, batch.pool_elems(), 4096)
-    valid = helpers.slot_valid_mask(batch, "ctx")
-    flat_valid = np.broadcast_to(valid[:, None, :, None], inp["k_pool"].shape).reshape(-1)[idx]
-    host = gen.bf16_normal_at(batch.seed, gen.TENSOR_K_POOL, idx.astype(np.uint64))
-    assert (inp["k_pool"].reshape(-1)[idx][flat_valid] == host[flat_valid]).all()
-    rng = np.random.default_rng(2)
-    rows = np.unique(np.concatenate([rng.integers(0, batch.n_tok, 96), [0, batch.n_tok - 1],
-                                     batch.cu_seqlens_q[:-1][-6:], batch.cu_seqlens_q[1:][-6:] - 1]))
-    ref, kp, vp = gc.run_oracle(batch, inp, rows=rows)
+    _device_pool_is_the_host_stream(batch, inp["k_pool"], gen.TENSOR_K_POOL)
+    ref, kp, vp = gc.run_oracle(batch, inp, n_threads=16)
     assert (sdev.bits(d["k_pool"]) == kp).all() and (sdev.bits(d["v_pool"]) == vp).all()
-    gc.check_close(sdev.bits(d["out"])[rows], ref, batch.name)
+    gc.check_close(sdev.bits(d["out"]), ref, f"{batch.name}/{order}")
 
 
 @pytest.mark.parametrize("ctx,r", [(128, 0.8), (64, 0.6), (256, 0.2), (512, 1.0)])
@@ -212,51 +306,78 @@ def test_table9_shaped_batches_parity(name, r):
     assert torch.isfinite(d["out"].float()).all()
 
 
-def test_config3_full_size_sampled():
+def test_config3_all_rows():
+    """C3 (Gemma-3-1B shape, 256 decode sequences): every output row vs the oracle, pools bit-exact."""
     batch = workloads.config3()
     d = gc.run_gpu(batch, None)
     inp = dict(q=batch.q_bits(), k_new=batch.kv_new_bits()[0], v_new=batch.kv_new_bits()[1],
                k_pool=sdev.bits(d["pool_before"][0]), v_pool=sdev.bits(d["pool_before"][1]))
-    rows = np.random.default_rng(3).choice(batch.n_tok, 48, replace=False)
-    ref, kp, vp = gc.run_oracle(batch, inp, rows=rows)
+    _device_pool_is_the_host_stream(batch, inp["v_pool"], gen.TENSOR_V_POOL, seed=4)
+    ref, kp, vp = gc.run_oracle(batch, inp, n_threads=16)
     assert (sdev.bits(d["k_pool"]) == kp).all() and (sdev.bits(d["v_pool"]) == vp).all()
-    gc.check_close(sdev.bits(d["out"])[rows], ref, batch.name)
-    got = gen.bf16_to_f64(sdev.bits(d["out"]))
-    assert np.isfinite(got).all()                       # property at full size: no sentinel leaked anywhere
+    gc.check_close(sdev.bits(d["out"]), ref, batch.name)
 
 
-def test_config4_full_size_sampled():
-    """C4 (Qwen3-8B shape, n_tok 8192) at r = 0.5, full size, in the launch configuration bench.py times: one mixed
-    launch over a ~40 GB pool; 96 sampled decode sequences + both prefill chunks (every 16th row) vs the oracle."""
+def _full_size_case(batch, n_decode_sample, seed, expect_mixed=None):
+    """Full-size configuration in the launch sequence bench.py times (plan, then append + attention).  Checks
+    (i) kv_append changed exactly its target slots: position-weighted checksums of BOTH whole pools before and after
+        (every other byte untouched, at full size), and the placement of the sampled sequences bit-exactly;
+    (ii) attention of >= 128 sampled decode sequences and of every 16th row (+ first/last) of every prefill chunk vs the
+        oracle; (iii) every output finite (no NaN sentinel leaked anywhere)."""
     import gc as pygc
     pygc.collect()
     torch.cuda.empty_cache()
-    batch = workloads.config4(0.5)
-    d = gc.run_gpu(batch, None)
-    rng = np.random.default_rng(45)
-    seqs = list(rng.choice(batch.num_decode_seqs, 96, replace=False)) + list(range(batch.num_decode_seqs, batch.n_seq))
-    gc.check_sampled_sequences(batch, d, seqs, what=batch.name)
-    assert torch.isfinite(d["out"].float()).all()      # property at full size: no NaN sentinel leaked anywhere
-    assert d["pa"].plan_info(6) > 0 and d["pa"].plan_info(1) > 0, "expected a mixed launch"
+    dev = "cuda:0"
+    w = gc._weights(dev)
+    state = {}
 
-
-def test_config5_full_size_sampled():
-    """C5 (Qwen3-30B-A3B shape, G = 8) with the 150 GB pool (3.75e10 elements per pool: 64-bit block addressing),
-    variant r0.2 (1024 decode sequences with ctx in [4096, 32768] + 4 prefill chunks of 1024)."""
-    import gc as pygc
-    pygc.collect()
-    torch.cuda.empty_cache()
-    free, _ = torch.cuda.mem_get_info()
-    nb = int(150e9 // (32 * 1024))
-    if free < 160e9:
-        nb = int((free - 8e9) // (32 * 1024))          # largest pool that fits this device (recorded in the test name)
-    batch = workloads.config5("r0.2", num_blocks=nb)
-    assert batch.block_tables.max() > (1 << 31) // (4 * 16 * 128), "block ids must reach past 2^31 elements"
-    d = gc.run_gpu(batch, None)
-    rng = np.random.default_rng(57)
-    seqs = list(rng.choice(batch.num_decode_seqs, 24, replace=False)) + list(range(batch.num_decode_seqs, batch.n_seq))
-    gc.check_sampled_sequences(batch, d, seqs, what=f"{batch.name}/nb={nb}")
+    def before(d):
+        tg = gc.append_targets(batch, dev)
+        state["tg"] = tg
+        for name in ("k", "v"):
+            pool = d[f"{name}_pool"]
+            state[name] = (gc.pool_checksum(pool, w), pool.view(-1)[tg.view(-1)].clone())
+    d = gc.run_gpu(batch, None, pre_append=before, keep_pool_copy=False)
+    for name in ("k", "v"):
+        c0, old = state[name]
+        want = gc.expected_checksum_after_append(c0, old, d[f"{name}_new"], state["tg"], w)
+        assert gc.pool_checksum(d[f"{name}_pool"], w) == want, f"{batch.name}: {name.upper()} pool changed outside the append targets"
+        assert (d[f"{name}_pool"].view(-1)[state["tg"].view(-1)].view(torch.int16) == d[f"{name}_new"].view(-1).view(torch.int16)).all()
+    rng = np.random.default_rng(seed)
+    nd = batch.num_decode_seqs
+    seqs = list(rng.choice(nd, min(nd, n_decode_sample), replace=False)) if nd else []
+    seqs += list(range(nd, batch.n_seq))
+    gc.check_sampled_sequences(batch, d, seqs, prefill_row_stride=16, n_threads=16, what=batch.name)
     assert torch.isfinite(d["out"].float()).all()
+    if expect_mixed is True:
+        assert d["pa"].plan_info(6) > 0 and d["pa"].plan_info(1) > 0, "expected a mixed launch"
+    return d
+
+
+@pytest.mark.parametrize("r", [0.0, 0.1, 0.5, 1.0])
+def test_config4_full_size_sampled(r):
+    """C4 (Qwen3-8B shape, n_tok 8192): r = 0 (2048-token chunks over prior context, the tensor-bound point), 0.1 and 0.5
+    (mixed launches) and 1.0 (8192 decode sequences, ~84 GB of KV) — PAPER.md:L62, L437, L508."""
+    batch = workloads.config4(r, num_blocks=workloads.c4_pool_blocks())       # the pool bench.py's headline loop uses
+    _full_size_case(batch, 128, 45 + int(10 * r), expect_mixed=(0 < r < 1) or None)
+
+
+@pytest.mark.parametrize("variant", ["r1.0", "r0.2", "r0.059"])
+def test_config5_full_size_sampled(variant):
+    """C5 (Qwen3-30B-A3B shape, G = 8) on the 150 GB pool (3.75e10 elements per pool: 64-bit block addressing); R15's three
+    variants.  Skips loudly when the device cannot hold the pool — it never shrinks it."""
+    import gc as pygc
+    pygc.collect()
+    torch.cuda.empty_cache()
+    nb = int(150e9 // (32 * 1024))
+    free, _ = torch.cuda.mem_get_info()
+    need = 2 * nb * 4 * 16 * 128 * 2 + 6e9
+    if free < need:
+        pytest.skip(f"C5 needs {need / 1e9:.0f} GB free for the 150 GB pool, device has {free / 1e9:.0f} GB")
+    batch = workloads.config5(variant, num_blocks=nb)
+    assert batch.num_blocks == int(150e9 // 32768)
+    assert batch.block_tables.max() > (1 << 31) // (4 * 16 * 128), "block ids must reach past 2^31 elements"
+    _full_size_case(batch, 128, 57, expect_mixed=(variant != "r1.0") or None)
 
 
 def test_empty_and_degenerate_batches():
