@@ -493,6 +493,9 @@ def _roofline(preps, K, attn_sec, app_sec, sec, peaks):
             "alg_bytes_per_launch": mean_bytes, "launch_us": mean_sec * 1e6,
             "kernel_share_of_step": float(np.sum(attn_sec)) / sec, "kv_append_share_of_step": float(np.sum(app_sec)) / sec,
             "roofline_time_frac": float(sum(r[0] for r in roofs) / np.sum(attn_sec)),
+            "per_r_launch_us": [float(np.mean([attn_sec[i] for i in range(K) if i % n == j])) * 1e6 for j in range(n)],
+            "per_r_roofline_frac": [float(np.sum([roofs[i][0] for i in range(K) if i % n == j]) /
+                                          np.sum([attn_sec[i] for i in range(K) if i % n == j])) for j in range(n)],
             "bound_note": "10 of the 11 r-batches are HBM-bound, r = 0 is tensor-bound (per_bound)", "per_bound": per_bound}
 
 

@@ -314,7 +314,7 @@ struct BundleCutter {
         cur += b1 - b0;
         ++n_items;
     }
-    void add_whole_sequence(int32_t grp0, int32_t groups, int32_t nblk) {   // `groups` consecutive groups, uncut
+    void add_whole_groups(int32_t grp0, int32_t groups, int32_t nblk) {   // `groups` consecutive groups of nblk blocks, uncut
         add(grp0, 0, nblk, nblk);
         if (overflow) return;
         out[n_bundles].grp_end = grp0 + groups - 1;
@@ -456,18 +456,21 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
         for (int s = 0; s < n_dec && !bc.overflow; ++s) {
             const int32_t nblk = (h_ctx[s] + kBlock) / kBlock;          // ceil((ctx + 1) / 16)
             const int32_t grp0 = s * Hkv;
-            if (bc.cur + (int64_t)Hkv * nblk < target) {
-                // every group of the sequence joins the open bundle whole and no boundary is reached
-                bc.add_whole_sequence(grp0, Hkv, nblk);
-                continue;
-            }
+            // a short group (<= 256 keys, or a quarter bundle) is never cut: partials + merge would cost more than
+            // the imbalance it leaves (a microsecond or two of streaming)
             const bool is_short = nblk <= 16 || (int64_t)nblk * 4 <= target;
-            for (int g = 0; g < Hkv && !bc.overflow; ++g) {
-                const int32_t grp = grp0 + g;
-                if (is_short && bc.cur + nblk > target) {
-                    // a short group (<= 256 keys, or a quarter bundle) is never cut: partials + merge would cost
-                    // more than the imbalance it leaves (a microsecond or two of streaming); it goes whole into this
-                    // bundle or the next, whichever ends nearer the target
+            for (int g = 0; g < Hkv && !bc.overflow;) {
+                // as many whole groups as fit the open bundle, in one step (the work is O(bundle boundaries))
+                const int32_t n_fit = (int32_t)std::min<int64_t>((target - bc.cur) / nblk, Hkv - g);
+                if (n_fit > 0) {
+                    bc.add_whole_groups(grp0 + g, n_fit, nblk);
+                    g += n_fit;
+                    if (bc.cur == target) bc.close();
+                    continue;
+                }
+                const int32_t grp = grp0 + g++;
+                if (is_short) {
+                    // goes whole into this bundle or the next, whichever ends nearer the target
                     if (bc.cur + nblk - target > target - bc.cur) bc.close();
                     bc.add(grp, 0, nblk, nblk);
                     if (bc.cur >= target) bc.close();

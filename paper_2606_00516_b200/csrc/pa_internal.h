@@ -52,7 +52,7 @@ static_assert(sizeof(PreTile) == 32, "PreTile layout");
 
 // Device-side view of the planned workspace (all pointers into the caller's workspace buffer).
 struct PlanView {
-    int32_t* queue;            // [0] next decode bundle, [1] exited CTAs, [2] next prefill unit, [3] rows to redo (all self-resetting)
+    int32_t* queue;            // [0] next decode bundle, [1] exited CTAs, [2] next prefill unit, [3] rows to redo (all self-resetting), [4] rows redone since pa_plan
     int32_t* group_counters;   // [num_decode_seqs * Hkv] arrivals of split groups (self-resetting)
     const DecBundle* bundles;  // [n_bundles] decode bundles
     int2* redo;                // prefill rows whose one-pass softmax overflowed: {tile index, (row in tile << 8) | q head}

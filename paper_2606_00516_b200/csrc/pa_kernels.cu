@@ -199,6 +199,7 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
             pl.queue[1] = 0;
             pl.queue[2] = 0;
             pl.queue[3] = 0;
+            pl.queue[4] += n_redo;      // cumulative since pa_plan: rows recomputed by the plain loop (introspection)
             __threadfence();
         }
     }

@@ -209,6 +209,8 @@ def test_prefill_overflow_rows_are_recomputed(shape_name, mode):
         else:
             inp["k_new"][row0 + t - ctx, :, 0] = v
     d = gc.run_gpu(batch, inp, flags=MODE_FLAGS[mode], repeat=2)        # repeat: the redo counter must self-reset
+    redone = int(d["pa"].workspace[:64].view(torch.int32)[4].item())    # workspace counter [4]: rows redone since pa_plan
+    assert redone >= 2 * 100 * shape.num_q_heads, f"expected the overflow rows to take the redo path, got {redone}"
     ref, _, _ = gc.run_oracle(batch, inp)
     gc.check_close(sdev.bits(d["out"]), ref, f"overflow/{shape_name}/mode{mode}")
 
