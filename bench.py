@@ -45,12 +45,18 @@ R_GRID = [i / 10 for i in range(11)]
 FIT_NTOK_C2 = [512, 1024, 2048, 4096]       # DESIGN R18
 FIT_NTOK_C4 = [2048, 4096, 8192]
 L2_FLUSH_BYTES = 512 << 20
-# dram__bytes_read.sum + dram__bytes_write.sum per pa_attention_kernel launch from OFFLINE `ncu --set full` captures
-# (profiles/, made with the committed command named there); the live line labels it as such.  None = no capture.
-NCU_TRAFFIC = {"workload": "C4 r-cycle", "bytes_per_launch": None, "source": None}
-_traffic_file = os.path.join(ROOT, "profiles", "r2_c4_traffic.json")
+# dram__bytes_read.sum + dram__bytes_write.sum per pa_attention_kernel launch from an OFFLINE ncu capture of the 11
+# launches of one C4 r-cycle (profiles/r2_c4_cycle_traffic.csv, made with the command named in the .md beside it);
+# the live line labels it as such.  No capture file = null.
+NCU_TRAFFIC = {"bytes_per_launch": None, "source": None}
+_traffic_file = os.path.join(ROOT, "profiles", "r2_c4_cycle_traffic.csv")
 if os.path.exists(_traffic_file):
-    NCU_TRAFFIC = json.load(open(_traffic_file))
+    import csv
+    with open(_traffic_file) as _f:
+        _rows = list(csv.DictReader(_f))
+    if _rows:
+        NCU_TRAFFIC = {"bytes_per_launch": sum(float(x["dram_read_bytes"]) + float(x["dram_write_bytes"]) for x in _rows) / len(_rows),
+                       "source": "profiles/r2_c4_cycle_traffic.csv (mean over the %d launches of one r-cycle)" % len(_rows)}
 
 
 def _peaks():

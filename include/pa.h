@@ -89,7 +89,8 @@ typedef struct {
     int32_t tune_prefill_ctas;        /* CTAs that start in the prefill role of a mixed launch (clamped to [1, SMs-1]) */
     int32_t tune_bundles_per_stream;  /* decode bundles per persistent stream, 1..4 */
     int32_t tune_min_bundle_blocks;   /* smallest decode bundle, in 16-token blocks (default 2) */
-    int32_t reserved;                 /* must be 0 */
+    int32_t tune_levels;              /* guided hand-out of decode bundles: pieces per bundle, 1..8 (1 = whole bundles);
+                                         effective value: pa_plan_info 10 */
 } pa_config;
 
 /* Create / destroy a context for one shape.  `out` host.  PA_ERR_UNSUPPORTED for shapes outside the
@@ -184,7 +185,8 @@ int32_t pa_crossover_eq7(const double* in, double* out);
  *        4 CTAs in the attention launch, 5 kernel launches per pa_batch_attention call,
  *        6 CTAs given the prefill role in the mixed launch, 7 decode bundles per stream (effective),
  *        8 prefill variant (0 P in TMEM, 1 P in shared memory, 2 plain kernel),
- *        9 host nanoseconds the last pa_plan call took (validation + lists + enqueue of the upload). */
+ *        9 host nanoseconds the last pa_plan call took (validation + lists + enqueue of the upload),
+ *        10 pieces a decode bundle is handed out in (guided hand-out; 1 = whole bundles). */
 int64_t pa_plan_info(const pa_ctx* ctx, int32_t which);
 
 /* Library-owned message of the last error on ctx (valid until the next call on ctx); "" if none. */

@@ -36,7 +36,7 @@ class PaConfig(C.Structure):
                 ("block_size", C.c_int32), ("num_blocks", C.c_int64), ("max_seqs", C.c_int32),
                 ("max_tokens", C.c_int32), ("max_blocks_per_seq", C.c_int32), ("device", C.c_int32),
                 ("flags", C.c_uint32), ("tune_prefill_ctas", C.c_int32), ("tune_bundles_per_stream", C.c_int32),
-                ("tune_min_bundle_blocks", C.c_int32), ("reserved", C.c_int32)]
+                ("tune_min_bundle_blocks", C.c_int32), ("tune_levels", C.c_int32)]
 
 
 _lib = None
@@ -106,11 +106,12 @@ class PagedAttention:
 
     def __init__(self, num_q_heads: int, num_kv_heads: int, head_dim: int, num_blocks: int, max_seqs: int,
                  max_tokens: int, max_blocks_per_seq: int, block_size: int = 16, device: int = 0, flags: int = 0,
-                 tune_prefill_ctas: int = 0, tune_bundles_per_stream: int = 0, tune_min_bundle_blocks: int = 0):
+                 tune_prefill_ctas: int = 0, tune_bundles_per_stream: int = 0, tune_min_bundle_blocks: int = 0,
+                 tune_levels: int = 0):
         self.lib = load_library()
         self.cfg = PaConfig(num_q_heads, num_kv_heads, head_dim, block_size, num_blocks, max_seqs, max_tokens,
                             max_blocks_per_seq, device, flags, tune_prefill_ctas, tune_bundles_per_stream,
-                            tune_min_bundle_blocks, 0)
+                            tune_min_bundle_blocks, tune_levels)
         self.ctx = C.c_void_p()
         rc = self.lib.pa_create(C.byref(self.ctx), C.byref(self.cfg))
         if rc != PA_OK:

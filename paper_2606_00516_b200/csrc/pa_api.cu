@@ -35,7 +35,7 @@ struct pa_ctx {
     bool planned = false;
     PlanView view{};
     int32_t decode_ctas = 0, n_simple_tiles = 0, launches_per_call = 0, prefill_ctas = 0, p_in_tmem = 1;
-    int32_t planned_n_tok = 0, n_items = 0, bundles_per_stream = 0, prefill_mode = 0;
+    int32_t planned_n_tok = 0, n_items = 0, bundles_per_stream = 0, prefill_mode = 0, n_levels = 1;
     int64_t plan_host_ns = 0;
     // tensor-map cache
     const void* tm_k_ptr = nullptr;
@@ -169,7 +169,7 @@ int32_t pa_create(pa_ctx** out, const pa_config* cfg) {
     if (cfg->num_q_heads <= 0 || cfg->num_kv_heads <= 0 || cfg->num_blocks <= 0 || cfg->max_seqs <= 0 ||
         cfg->max_tokens <= 0 || cfg->max_blocks_per_seq <= 0 || cfg->device < 0 || cfg->tune_prefill_ctas < 0 ||
         cfg->tune_bundles_per_stream < 0 || cfg->tune_bundles_per_stream > 4 || cfg->tune_min_bundle_blocks < 0 ||
-        cfg->reserved != 0)
+        cfg->tune_levels < 0 || cfg->tune_levels > 8)
         return PA_ERR_INVALID;
     if ((cfg->head_dim != 128 && cfg->head_dim != 256) || cfg->block_size != kBlock ||
         cfg->num_q_heads % cfg->num_kv_heads != 0 || cfg->num_q_heads / cfg->num_kv_heads > kMaxGroup)
@@ -437,7 +437,7 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     // ---- decode bundles
     const int64_t off_b = align_up((int64_t)n_tiles * sizeof(PreTile), 256);
     BundleCutter bc{reinterpret_cast<DecBundle*>(h_stage + off_b), ctx->max_bundles, ctx->max_split, 1};
-    int k = 0;
+    int k = 0, levels = 1;
     if (total_blocks > 0) {
         // workers that start in the decode role; in a mixed launch the prefill CTAs join through the queue when
         // their units run out, so bundles are made finer (>= 2 per worker) and the tail balances dynamically
@@ -449,6 +449,15 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
         // queue-drawn bundle per worker evens out unequal stream rates (C5: -5 %).  Mixed launches: 2 per worker.
         const double kv_bytes = (double)total_blocks * kBlock * D * 2 * 2;
         k = (mixed || kv_bytes >= 16e9) ? 2 : 1;
+        // Guided hand-out (PlanView::n_levels): when a stream's share holds many groups (>= 16) and the launch is long
+        // enough for unequal stream rates to matter (>= 1 GB of KV, ~150 us), ONE bundle per stream is taken in eight
+        // pieces of 50, 20, 12, 7, 5, 3, 2, 1 % of its groups: with equal bundles every stream ends up with exactly
+        // k of them and the launch ends with its slowest stream (measured on C4: 7-12 % behind the mean).  Pieces are
+        // whole groups, so no group is cut more often, and the planner does no extra work.
+        const double groups_per_share = (double)n_dec * Hkv / (double)W;
+        levels = (groups_per_share >= 16.0 && kv_bytes >= 1e9) ? 8 : 1;
+        if (c.tune_levels > 0) levels = c.tune_levels;
+        if (levels > 1) k = 1;
         if (c.tune_bundles_per_stream > 0) k = c.tune_bundles_per_stream;
         const int64_t min_blocks = c.tune_min_bundle_blocks > 0 ? c.tune_min_bundle_blocks : 2;
         const int64_t target = std::max(min_blocks, (total_blocks + W * k - 1) / (W * k));
@@ -458,10 +467,16 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
             const int32_t grp0 = s * Hkv;
             // a short group (<= 256 keys, or a quarter bundle) is never cut: partials + merge would cost more than
             // the imbalance it leaves (a microsecond or two of streaming)
+            if (bc.cur + (int64_t)nblk * Hkv < target) {        // the whole sequence joins the open bundle
+                bc.add_whole_groups(grp0, Hkv, nblk);
+                continue;
+            }
             const bool is_short = nblk <= 16 || (int64_t)nblk * 4 <= target;
             for (int g = 0; g < Hkv && !bc.overflow;) {
                 // as many whole groups as fit the open bundle, in one step (the work is O(bundle boundaries))
-                const int32_t n_fit = (int32_t)std::min<int64_t>((target - bc.cur) / nblk, Hkv - g);
+                const int64_t room = target - bc.cur;
+                const int32_t n_fit = room < nblk ? 0 : (int32_t)std::min<int64_t>(
+                    room < (int64_t(1) << 31) ? (int64_t)((uint32_t)room / (uint32_t)nblk) : room / nblk, Hkv - g);
                 if (n_fit > 0) {
                     bc.add_whole_groups(grp0 + g, n_fit, nblk);
                     g += n_fit;
@@ -517,6 +532,16 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     v.n_split = bc.n_split;
     v.n_units = n_units;
     v.head_groups = head_groups;
+    {   // cumulative shares of the pieces in 1/256 (the last one is stored as 255 and read as 256)
+        static const uint8_t kCum8[8] = {128, 179, 210, 228, 241, 249, 254, 255};
+        uint64_t cum = 0;
+        for (int l = 1; l <= levels; ++l) {
+            const uint64_t cv = (l == levels) ? 255 : (levels == 8 ? kCum8[l - 1] : (uint64_t)(256 * l / levels));
+            cum |= cv << (8 * (l - 1));
+        }
+        v.n_levels = levels;
+        v.level_cum = cum;
+    }
     int32_t dec_ctas = 0;
     if (n_bundles > 0) dec_ctas = std::min(sms - pre_ctas, n_bundles);
     ctx->decode_ctas = dec_ctas;
@@ -524,6 +549,7 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     ctx->p_in_tmem = prefill_mode == 0;
     ctx->prefill_mode = prefill_mode;
     ctx->bundles_per_stream = k;
+    ctx->n_levels = levels;
     ctx->n_items = bc.n_items;
     ctx->n_simple_tiles = prefill_mode == 2 ? n_tiles : 0;
     ctx->planned_n_tok = n_tok;
@@ -600,6 +626,10 @@ int64_t pa_plan_info(const pa_ctx* ctx, int32_t which) {
         case 7: return ctx->bundles_per_stream;
         case 8: return ctx->prefill_mode;
         case 9: return ctx->plan_host_ns;
+        case 10: return ctx->n_levels;
+#ifdef PA_TIMELINE
+        case 100: return ctx->off_redo;     // development instrumentation (pa_prefill.cuh PA_TL)
+#endif
         default: return PA_ERR_INVALID;
     }
 }

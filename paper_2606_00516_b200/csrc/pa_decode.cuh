@@ -91,24 +91,44 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
     // comes from the queue.  The queue index is requested two bundles ahead and the 32-byte descriptor one bundle
     // ahead of their use, so neither the atomic nor the descriptor load is waited on where it is issued.
     const int4* bundles = reinterpret_cast<const int4*>(pl.bundles);
+    // tickets: level-major (PlanView::n_levels); ticket -> (level, bundle)
+    const int n_tickets = pl.n_bundles * pl.n_levels;
+    auto ticket_bundle = [&](int ticket, int& level) -> int {
+        level = 0;
+        if (pl.n_levels > 1) { level = ticket / pl.n_bundles; ticket -= level * pl.n_bundles; }
+        return ticket;
+    };
+    auto level_cum = [&](int l) -> int { return l == 0 ? 0 : (int)((pl.level_cum >> (8 * (l - 1))) & 0xffu) + (l == pl.n_levels ? 1 : 0); };
     int b_next = first_bundle;
     if (b_next < 0) b_next = p.decode_workers + atomicAdd(&pl.queue[0], 1);
-    int4 nd0 = make_int4(0, 0, -1, 0), nd1 = nd0;        // descriptor of bundle b_next
-    bool have_next = b_next < pl.n_bundles;
-    if (have_next) { nd0 = __ldg(bundles + 2 * b_next); nd1 = __ldg(bundles + 2 * b_next + 1); }
-    int b_after = have_next ? p.decode_workers + atomicAdd(&pl.queue[0], 1) : pl.n_bundles;
+    int4 nd0 = make_int4(0, 0, -1, 0), nd1 = nd0;        // descriptor of the bundle of ticket b_next
+    int lvl_next = 0;
+    bool have_next = b_next < n_tickets;
+    if (have_next) {
+        const int bb = ticket_bundle(b_next, lvl_next);
+        nd0 = __ldg(bundles + 2 * bb); nd1 = __ldg(bundles + 2 * bb + 1);
+    }
+    int b_after = have_next ? p.decode_workers + atomicAdd(&pl.queue[0], 1) : n_tickets;
     int4 d0 = make_int4(0, 0, -1, 0), d1 = d0;           // current bundle: {grp_begin, blk_begin, grp_end, blk_end}, parts
     int grp = 0, grp_last = -1;
     // A group of the walk, with its context length in flight: {seq, kv head, blk_begin, blk_end or -1}, {ctx, part_base, part}
     auto next_group = [&](int4& ga, int4& gb) -> bool {
-        if (grp > grp_last) {
+        while (grp > grp_last) {
             if (!have_next) return false;
             d0 = nd0; d1 = nd1;
-            grp = d0.x; grp_last = d0.z;
-            have_next = b_after < pl.n_bundles;
+            const int lvl = lvl_next;
+            have_next = b_after < n_tickets;
             if (have_next) {
-                nd0 = __ldg(bundles + 2 * b_after); nd1 = __ldg(bundles + 2 * b_after + 1);
+                const int bb = ticket_bundle(b_after, lvl_next);
+                nd0 = __ldg(bundles + 2 * bb); nd1 = __ldg(bundles + 2 * bb + 1);
                 b_after = p.decode_workers + atomicAdd(&pl.queue[0], 1);
+            }
+            if (pl.n_levels > 1) {
+                const int n = d0.z - d0.x + 1;           // groups of the bundle; this ticket takes its piece `lvl`
+                grp = d0.x + ((n * level_cum(lvl)) >> 8);
+                grp_last = d0.x + ((n * level_cum(lvl + 1)) >> 8) - 1;      // empty piece: try the next ticket
+            } else {
+                grp = d0.x; grp_last = d0.z;
             }
         }
         const int seq = grp / p.Hkv, kvh = grp - seq * p.Hkv;

@@ -62,6 +62,13 @@ struct PlanView {
     int32_t n_items, n_bundles, n_tiles, n_split;
     int32_t n_units;           // prefill work units = n_tiles * Hkv * head_groups (tcgen05 path; 0 = none)
     int32_t head_groups;       // ceil(G / q-tiles per CTA): units per (tile, KV head)
+    // Guided hand-out of decode bundles: a bundle of n groups is taken in n_levels pieces, piece l = the groups
+    // [n * cum[l] / 256, n * cum[l + 1] / 256) of the bundle (cum[0] = 0, cum[n_levels] = 256; cum[1..8] packed one byte
+    // each into level_cum).  The queue hands out tickets = level * n_bundles + bundle, level-major, so every stream
+    // starts with the large first piece of its own bundle and the small late pieces even out unequal stream rates at
+    // no cost to the planner and without cutting any more groups.  n_levels = 1: a ticket is a whole bundle.
+    int32_t n_levels;
+    uint64_t level_cum;
 };
 
 }  // namespace pa

@@ -139,7 +139,7 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
     const PlanView& pl = p.plan;
     // set-up spread over threads (it is on the critical path of microsecond-scale launches): thread 0 the prefill
     // barriers, threads 32.. one decode stream each, thread 64 the descriptor prefetches
-    if (threadIdx.x == 0 && pl.n_units > 0) prefill_init_barriers(ctrl);
+    if (threadIdx.x == 0 && pl.n_units > 0) prefill_init_barriers(ctrl, PrefillCfg<D, kPinTmem>::NQ);
     if (threadIdx.x >= 32 && threadIdx.x < 32 + kDecodeWarps && pl.n_bundles > 0)
         decode_init_barriers<D>(dec_aux, (int)threadIdx.x - 32);
     if (threadIdx.x == 64) {
@@ -170,7 +170,7 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
             if (pl.n_units > 0 && (starts_prefill || pl.n_units > p.prefill_ctas))
                 prefill_role<D, kPinTmem>(p, &tmQ, &tmK, &tmV, tiles, ctrl, starts_prefill ? (int)blockIdx.x : -1);
         } else {
-            if (pl.n_bundles > 0 && (!starts_prefill || pl.n_bundles > p.decode_workers))
+            if (pl.n_bundles > 0 && (!starts_prefill || pl.n_bundles * pl.n_levels > p.decode_workers))
                 decode_role<D>(p, &tmQd, &tmK, &tmV, &tails, tiles, dec_aux, starts_prefill ? -1 : dec_rank);
         }
         __syncthreads();

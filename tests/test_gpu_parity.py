@@ -115,7 +115,8 @@ def test_call_orders_small(name, order):
 
 @pytest.mark.parametrize("tune", [dict(tune_prefill_ctas=1), dict(tune_prefill_ctas=100), dict(tune_bundles_per_stream=4),
                                   dict(tune_bundles_per_stream=1, tune_min_bundle_blocks=1),
-                                  dict(tune_min_bundle_blocks=64)])
+                                  dict(tune_min_bundle_blocks=64), dict(tune_levels=8), dict(tune_levels=3, tune_bundles_per_stream=2),
+                                  dict(tune_levels=8, tune_min_bundle_blocks=64)])
 def test_planner_knobs_change_the_schedule_not_the_result(tune):
     """pa_config.tune_* (the documented replacements of round 1's environment variables): any setting is a valid plan."""
     batch = _small_case("ragged-g4-d128")
@@ -126,12 +127,28 @@ def test_planner_knobs_change_the_schedule_not_the_result(tune):
         assert d["pa"].plan_info(6) == min(tune["tune_prefill_ctas"], 147, d["pa"].plan_info(3) * 8 * 2)
     if "tune_bundles_per_stream" in tune:
         assert d["pa"].plan_info(7) == tune["tune_bundles_per_stream"]
+    if "tune_levels" in tune:
+        assert d["pa"].plan_info(10) == tune["tune_levels"]
     gc.check_close(sdev.bits(d["out"]), ref, f"knobs/{tune}")
     long = workloads.make_batch("split", workloads.GEMMA3_1B, 209, [1, 1, 1], [5000, 3333, 4097], 3)
     inp = helpers.host_inputs(long)
     ref, _, _ = gc.run_oracle(long, inp)
     d = gc.run_gpu(long, inp, tune=tune, repeat=2)
     gc.check_close(sdev.bits(d["out"]), ref, f"knobs-long/{tune}")
+
+
+@pytest.mark.parametrize("levels", [2, 8])
+@pytest.mark.parametrize("r", [0.5, 1.0])
+def test_guided_handout_many_groups_per_bundle(r, levels):
+    """Guided hand-out (pa_config.tune_levels, PlanView::n_levels): bundles of many short groups taken piece by piece,
+    every row against the oracle, twice on one plan (tickets and queue reset).  min_bundle_blocks makes the bundles long."""
+    batch = workloads.config2(r, n_tok=1024, ctx=40)
+    inp = helpers.host_inputs(batch)
+    ref, kp, vp = gc.run_oracle(batch, inp)
+    d = gc.run_gpu(batch, inp, tune=dict(tune_levels=levels, tune_min_bundle_blocks=96), repeat=2)
+    assert d["pa"].plan_info(10) == levels
+    assert (sdev.bits(d["k_pool"]) == kp).all() and (sdev.bits(d["v_pool"]) == vp).all()
+    gc.check_close(sdev.bits(d["out"]), ref, f"guided/r{r}/L{levels}")
 
 
 @pytest.mark.parametrize("name", ["C1", "ragged-g4-d128", "ragged-g4-d256"])
