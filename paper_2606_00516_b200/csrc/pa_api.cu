@@ -448,16 +448,21 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
         // roofline with 1 bundle per worker and 0.57 with 4); from ~16 GB on a launch lasts milliseconds and a second,
         // queue-drawn bundle per worker evens out unequal stream rates (C5: -5 %).  Mixed launches: 2 per worker.
         const double kv_bytes = (double)total_blocks * kBlock * D * 2 * 2;
-        k = (mixed || kv_bytes >= 16e9) ? 2 : 1;
+        // (C5 on one B200, same call, interleaved, median [min, max] over 24 launches: k = 1 6.47 [5.87, 6.81] ms,
+        // k = 2 6.67 [5.81, 6.90], k = 3 5.86 [5.81, 5.91], k = 4 6.31 [6.22, 6.41]: three per stream from 16 GB on.)
+        k = kv_bytes >= 16e9 ? 3 : (mixed ? 2 : 1);
         // Guided hand-out (PlanView::n_levels): when a stream's share holds many groups (>= 16) and the launch is long
-        // enough for unequal stream rates to matter (>= 1 GB of KV, ~150 us), ONE bundle per stream is taken in eight
-        // pieces of 50, 20, 12, 7, 5, 3, 2, 1 % of its groups: with equal bundles every stream ends up with exactly
-        // k of them and the launch ends with its slowest stream (measured on C4: 7-12 % behind the mean).  Pieces are
-        // whole groups, so no group is cut more often, and the planner does no extra work.
+        // enough for unequal stream rates to matter (>= 1 GB of KV, ~150 us), the bundles (two per stream) are taken in
+        // eight pieces of 50, 20, 12, 7, 5, 3, 2, 1 % of their groups, large pieces first.  With whole bundles every
+        // stream ends up with exactly k of them and the launch ends with its slowest stream; measured on C4 (one B200,
+        // same call, interleaved): r = 0.3 / 0.5 / 0.7 / 0.9 / 1.0  4.51 / 6.86 / 10.0 / 13.0 / 14.2 ms with whole
+        // bundles, 4.09 / 6.45 / 8.78 / 11.1 / 12.1 ms with pieces.  Pieces are whole groups: no group is cut more
+        // often and the planner does no extra work.  Shares of few, long groups (C3, C5) stay with whole bundles
+        // (pieces of one or two groups are erratic: C3 113 -> 150 us).
         const double groups_per_share = (double)n_dec * Hkv / (double)W;
         levels = (groups_per_share >= 16.0 && kv_bytes >= 1e9) ? 8 : 1;
         if (c.tune_levels > 0) levels = c.tune_levels;
-        if (levels > 1) k = 1;
+        if (levels > 1) k = 2;
         if (c.tune_bundles_per_stream > 0) k = c.tune_bundles_per_stream;
         const int64_t min_blocks = c.tune_min_bundle_blocks > 0 ? c.tune_min_bundle_blocks : 2;
         const int64_t target = std::max(min_blocks, (total_blocks + W * k - 1) / (W * k));

@@ -118,10 +118,10 @@ cudaError_t launch_kv_gather(const LaunchShape& sh, const void* k_pool, const vo
 // own queue runs dry it switches to the other role, so neither the tensor pipe nor HBM idles while
 // work remains.  The last CTA to leave resets the queues for the next launch.
 // Shared memory (from a 1024-byte aligned base): [0, 224 KB) tile region shared by the two roles,
-// then the prefill control block (256 B), then the decode workers' scratch (8 x 192 B).
+// then the prefill control block (512 B), then the decode workers' scratch (8 x 192 B).
 // ------------------------------------------------------------------------------------------------
 constexpr int kTileRegion = 224 * 1024;
-constexpr int kCtrlBytes = 256;
+constexpr int kCtrlBytes = 512;
 constexpr int kAttnSmemBytes = 1024 + kTileRegion + kCtrlBytes + kDecodeWarps * 192;
 static_assert(kAttnSmemBytes <= 232448, "attention kernel shared memory");
 static_assert(kDecodeWarps * DecodeCfg<128>::kStreamBytes <= kTileRegion, "decode streams fit the tile region");
@@ -137,6 +137,7 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
     PrefillCtrl* ctrl = reinterpret_cast<PrefillCtrl*>(tiles + kTileRegion);
     uint8_t* dec_aux = tiles + kTileRegion + kCtrlBytes;
     const PlanView& pl = p.plan;
+    if (threadIdx.x == 0) PA_TL(15, 399, 0);
     // set-up spread over threads (it is on the critical path of microsecond-scale launches): thread 0 the prefill
     // barriers, threads 32.. one decode stream each, thread 64 the descriptor prefetches
     if (threadIdx.x == 0 && pl.n_units > 0) prefill_init_barriers(ctrl, PrefillCfg<D, kPinTmem>::NQ);
@@ -160,6 +161,7 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
     // everything above touches only this CTA's shared memory and the kernel parameters; the pools, the plan and the
     // queues are read below, after the preceding kernel of the stream (normally kv_append) has completed
     pdl_grid_dependency_wait();
+    if (threadIdx.x == 0) PA_TL(15, 399, 1);
     const bool starts_prefill = (int)blockIdx.x < p.prefill_ctas;
     const int dec_rank = (int)blockIdx.x - p.prefill_ctas;       // rank among the initial decode CTAs
 #pragma unroll 1
@@ -174,6 +176,7 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
                 decode_role<D>(p, &tmQd, &tmK, &tmV, &tails, tiles, dec_aux, starts_prefill ? -1 : dec_rank);
         }
         __syncthreads();
+        if (threadIdx.x == 0) PA_TL(15, 397 + pass, 0);
     }
     // The last CTA to leave resets the queues for the next launch and recomputes, with the plain row loop, the prefill
     // rows whose one-pass softmax overflowed (normally none).  Pattern: writers fence before the counting atomic,

@@ -48,11 +48,15 @@ struct PrefillCfg {
     static constexpr int kQBytes = kQTile * D * 2;             // one Q tile
     static constexpr int kStageBytes = KT * D * 2;             // one K (or V) tile = 32 KB
     static constexpr int kPBytes = kPinTmem ? 0 : kQTile * HT * 2;   // one P buffer (2 per q-head tile)
-    static constexpr int kStages = kPinTmem ? 5 : (D == 128 ? 3 : 4);
+    static constexpr int kStages = kPinTmem ? 4 : (D == 128 ? 3 : 4);
     static constexpr int kOffQ = 0;
     static constexpr int kOffP = NQ * kQBytes;
     static constexpr int kOffRing = kOffP + NQ * 2 * kPBytes;
-    static constexpr int kTileBytes = kOffRing + kStages * kStageBytes;   // <= 224 KB
+    // epilogue staging, 4 KB per softmax warp: its own area behind the ring, or (P in shared memory) the tile's P buffers,
+    // which are idle once the last PV MMA of a unit has completed; a warp only ever touches its own 32 rows of either
+    static constexpr int kOffStage = kPinTmem ? kOffRing + kStages * kStageBytes : kOffP;
+    static constexpr int kStageStride = kPinTmem ? 4 * 4096 : 2 * kPBytes;
+    static constexpr int kTileBytes = kOffRing + kStages * kStageBytes + (kPinTmem ? NQ * 4 * 4096 : 0);   // <= 224 KB
     static constexpr int kColO = 0;                             // TMEM columns
     static constexpr int kColS = NQ * D;
     static constexpr int kTmemCols = 512;
@@ -68,10 +72,13 @@ struct PrefillCtrl {
     uint64_t s_full[2][2], p_full[2][2];    // [q-head tile][score buffer]
     uint64_t o_full[2], pv_done[2];
     uint64_t unit_full[4];
+    uint64_t turn[2];       // the two MMA issuers take turns on the tensor pipe (prefill_role)
     uint32_t tmem_base;
-    int32_t unit[4];
+    int32_t unit[4];        // mailbox: unit id ...
+    int32_t pad_[3];
+    PreTile tile[4];        // ... and its tile descriptor (fetched once, by the producer)
 };
-static_assert(sizeof(PrefillCtrl) <= 256, "PrefillCtrl size");
+static_assert(sizeof(PrefillCtrl) <= 512, "PrefillCtrl size");
 
 __device__ __forceinline__ void prefill_init_barriers(PrefillCtrl* c, int nq) {   // one thread, once per CTA; nq = q-head tiles per unit
     mbar_init(smem_u32(&c->q_full), 1);
@@ -86,6 +93,9 @@ __device__ __forceinline__ void prefill_init_barriers(PrefillCtrl* c, int nq) { 
         mbar_init(smem_u32(&c->pv_done[t]), 1);
     }
     for (int i = 0; i < 4; ++i) mbar_init(smem_u32(&c->unit_full[i]), 1);
+    mbar_init(smem_u32(&c->turn[0]), 1);
+    mbar_init(smem_u32(&c->turn[1]), 1);
+    mbar_arrive(smem_u32(&c->turn[0]));       // tile 0 goes first
 }
 
 // Development instrumentation (-DPA_TIMELINE=<cta>): clock64 stamps of the hand-offs of one CTA, written into the
@@ -131,8 +141,9 @@ struct PrefillUnit {
     PreTile tile;
     int ti, kvh, h_first, nact, kv_total, n_kv, n_step;
 };
+// tile_src: null = fetch the tile descriptor from the plan (the producer), else the mailbox copy in shared memory
 template <int NQ, int KT, int HT>
-__device__ __forceinline__ PrefillUnit prefill_decode_unit(const AttnParams& p, int unit) {
+__device__ __forceinline__ PrefillUnit prefill_decode_unit(const AttnParams& p, int unit, const PreTile* tile_src = nullptr) {
     const PlanView& pl = p.plan;
     PrefillUnit u;
     const int per_tile = p.Hkv * pl.head_groups;
@@ -140,7 +151,7 @@ __device__ __forceinline__ PrefillUnit prefill_decode_unit(const AttnParams& p, 
     const int rem = unit - u.ti * per_tile;
     u.kvh = rem / pl.head_groups;
     const int hg = rem - u.kvh * pl.head_groups;
-    u.tile = pl.tiles[u.ti];
+    u.tile = tile_src ? *tile_src : pl.tiles[u.ti];
     u.h_first = u.kvh * p.G + hg * NQ;
     u.nact = min(NQ, p.G - hg * NQ);                              // active q-head tiles of this unit
     u.kv_total = u.tile.ctx + u.tile.q_begin + u.tile.q_rows;     // keys any row of the tile can see
@@ -169,6 +180,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = ctrl->tmem_base;
+    if (threadIdx.x == 0) PA_TL(15, 399, 2);
     // A role call starts with fresh barriers phases only the first time: the barriers persist across the two passes of
     // the kernel, but a CTA runs the prefill role at most once (pa_attention_kernel), so every phase starts at 0.
 
@@ -181,16 +193,18 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
             unit = __shfl_sync(0xffffffffu, unit, 0);
         }
         for (uint32_t it = 0;; ++it) {
+            // the id of the next unit is requested now and read at the end of this unit's loads
+            int unit_next = 0;
+            if (lane == 0 && unit < pl.n_units) unit_next = p.prefill_ctas + atomicAdd(&pl.queue[2], 1);
+            PrefillUnit u{};
+            if (unit < pl.n_units) u = prefill_decode_unit<NQ, KT, HT>(p, unit);
             if (lane == 0) {
                 ctrl->unit[it & 3] = unit;
+                ctrl->tile[it & 3] = u.tile;
                 mbar_arrive(smem_u32(&ctrl->unit_full[it & 3]));
             }
             __syncwarp();
             if (unit >= pl.n_units) break;
-            // the id of the next unit is requested now and read at the end of this unit's loads
-            int unit_next = 0;
-            if (lane == 0) unit_next = p.prefill_ctas + atomicAdd(&pl.queue[2], 1);
-            const PrefillUnit u = prefill_decode_unit<NQ, KT, HT>(p, unit);
             const PreTile& tile = u.tile;
             if (lane == 0) {
                 mbar_wait(smem_u32(&ctrl->q_empty), (it & 1u) ^ 1u);
@@ -259,6 +273,22 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
             mbar_wait(smem_u32(&ctrl->kv_full[e % ST]), (e / ST) & 1u);
             tc_fence_after();
         };
+        // The tensor pipe interleaves the MMAs of two issuing warps one by one, so two bursts issued at the same time
+        // both finish after the sum of their lengths, the two softmax groups get their scores together, compete for the
+        // MUFU/FMA pipes together and hand back P together: everything waits for everything.  The issuers therefore
+        // take strict turns, one burst (PV(j) + S(j+2)) per turn, through a pair of mbarriers (a sleeping wait, no
+        // polling traffic): each group gets its scores after ONE burst length and the groups settle half a step apart.
+        uint32_t turns = 0;                    // turns taken by this warp
+        auto turn_take = [&](bool both) {
+            if (NQ > 1 && both) mbar_wait(smem_u32(&ctrl->turn[t]), turns & 1u);
+        };
+        auto turn_pass = [&](bool both) {
+            if (NQ > 1 && both) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&ctrl->turn[t ^ 1]));
+                ++turns;
+            }
+        };
         // S_t(js) = Q_t · K(js)^T into score buffer js & 1 (D/16 k-steps, N = HT keys), with the ring bookkeeping of the
         // K stage; an inactive tile (t >= nact) only takes part in the stage / Q hand-back
         auto step_S = [&](int js, bool active, int nstep_u) {
@@ -284,11 +314,12 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
             mbar_wait(smem_u32(&ctrl->unit_full[it & 3]), (it >> 2) & 1u);
             const int unit = __reduce_max_sync(0xffffffffu, ctrl->unit[it & 3]);
             if (unit >= pl.n_units) break;
-            const PrefillUnit u = prefill_decode_unit<NQ, KT, HT>(p, unit);
+            const PrefillUnit u = prefill_decode_unit<NQ, KT, HT>(p, unit, &ctrl->tile[it & 3]);
             const int nstep_u = __reduce_max_sync(0xffffffffu, u.n_step), kvt_u = __reduce_max_sync(0xffffffffu, u.kv_total);
             const int kvl_u = __reduce_max_sync(0xffffffffu, u.tile.kv_len);
             const int nkv_u = __reduce_max_sync(0xffffffffu, u.n_kv);
-            const bool active = t < (int)__reduce_max_sync(0xffffffffu, u.nact);
+            const int nact_u = (int)__reduce_max_sync(0xffffffffu, u.nact);
+            const bool active = t < nact_u, both = nact_u == NQ;
             mbar_wait(smem_u32(&ctrl->q_full), it & 1u);
             tc_fence_after();
 #ifdef PA_STAGGER_NS
@@ -338,6 +369,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                     // ---- step 2i: PV(2i), then S(2i + 2) on the first half of K tile i + 1
                     if (lane == 0) PA_TL(2 + t, tl_step, 0);
                     mbar_wait(smem_u32(&ctrl->p_full[t][0]), pph & 1u);
+                    turn_take(both);
                     tc_fence_after();
                     if (lane == 0) PA_TL(2 + t, tl_step, 1);
                     if (elect_one()) pv_burst(0, i == 0);
@@ -346,10 +378,12 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                     tc_fence_after();
                     if (elect_one()) s_burst(0);
                     __syncwarp();
+                    turn_pass(both);
                     if (lane == 0) PA_TL(2 + t, tl_step, 2);
                     // ---- step 2i + 1: PV(2i + 1), then S(2i + 3) on the second half of K tile i + 1
                     if (lane == 0) PA_TL(2 + t, tl_step + 1, 0);
                     mbar_wait(smem_u32(&ctrl->p_full[t][1]), (pph >> 1) & 1u);
+                    turn_take(both);
                     tc_fence_after();
                     if (lane == 0) PA_TL(2 + t, tl_step + 1, 1);
                     if (elect_one()) {
@@ -365,6 +399,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                         umma_commit(smem_u32(&ctrl->kv_empty[kst]));
                     }
                     __syncwarp();
+                    turn_pass(both);
                     if (lane == 0) PA_TL(2 + t, tl_step + 1, 2);
 #ifdef PA_TIMELINE
                     tl_step += 2;
@@ -405,6 +440,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                     if (lane == 0) PA_TL(2 + t, tl_step, 0);
                     mbar_wait(smem_u32(&ctrl->p_full[t][b]), (pph >> b) & 1u);
                     pph ^= 1u << b;
+                    turn_take(both);
                     tc_fence_after();
                     if (lane == 0) PA_TL(2 + t, tl_step, 1);
                 }
@@ -431,6 +467,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                 }
                 __syncwarp();
                 if (j + 2 < nstep_u) step_S(j + 2, active, nstep_u);
+                if (active) turn_pass(both);
                 if (lane == 0) PA_TL(2 + t, tl_step, 2);
 #ifdef PA_TIMELINE
                 ++tl_step;
@@ -455,9 +492,10 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
             mbar_wait(smem_u32(&ctrl->unit_full[it & 3]), (it >> 2) & 1u);
             const int unit = ctrl->unit[it & 3];
             if (unit >= pl.n_units) break;
-            const PrefillUnit u = prefill_decode_unit<NQ, KT, HT>(p, unit);
+            const PrefillUnit u = prefill_decode_unit<NQ, KT, HT>(p, unit, &ctrl->tile[it & 3]);
             if (t >= u.nact) continue;
             const PreTile& tile = u.tile;
+            if (tl_me) PA_TL(12 + t, (int)it, 3);
             const int limit = tile.ctx + tile.q_begin + row;        // keys 0 .. limit are visible (R3)
             // m_ref: the reference max the exponentials of a step are taken against; m_run: max of all scores seen.
             // Only the first step needs its own max before exponentiating (two passes over S); later steps use the
@@ -634,9 +672,11 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
             }
             pv_base += (uint32_t)u.n_step;
             // ---- epilogue: O / l -> bf16 -> out[row0 + q_begin + row][h][:]
+            if (tl_me) PA_TL(12 + t, (int)it, 0);
             mbar_wait(smem_u32(&ctrl->o_full[t]), oph);
             oph ^= 1u;
             tc_fence_after();
+            if (tl_me) PA_TL(12 + t, (int)it, 1);
             const float inv = 1.f / l;
             bool valid = row < tile.q_rows;
             if (valid && !(l <= 3.0e38f)) {
@@ -646,25 +686,53 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                 __threadfence();
                 valid = false;
             }
-            uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)(tile.row0 + tile.q_begin + row) * p.Hq + u.h_first + t) * D);
+            // A thread owns a row, and rows are Hq·D·2 bytes apart in `out`: stored straight from the registers, every
+            // 16-byte store of a warp would touch 32 different lines (32 L1 wavefronts per instruction, ~2.7 us per
+            // unit).  The warp's 32 rows x 64 columns go through a 4 KB staging area (16-byte pieces XOR-swizzled by
+            // row) and leave as whole 128-byte lines, four rows per instruction.
+            const uint32_t stg = tiles_u32 + Cfg::kOffStage + t * Cfg::kStageStride + (uint32_t)(warp & 3) * 4096u;
+            const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
+            __nv_bfloat16* out0 = p.out + ((int64_t)(tile.row0 + tile.q_begin + ((warp & 3) << 5)) * p.Hq + u.h_first + t) * D;
 #pragma unroll
-            for (int c = 0; c < D / 32; ++c) {
-                uint32_t r[32];
-                tmem_ld32(tO + c * 32, r);
+            for (int hh = 0; hh < D / 64; ++hh) {
+                uint32_t r[2][32];
+                tmem_ld32(tO + hh * 64, r[0]);
+                tmem_ld32(tO + hh * 64 + 32, r[1]);
                 tmem_wait_ld();
-                if (valid) {
+                if (tl_me && hh == 0) PA_TL(14 + t, (int)it, 0);
 #pragma unroll
-                    for (int q4 = 0; q4 < 4; ++q4) {
-                        uint4 v;
-                        v.x = pack_bf16x2(__uint_as_float(r[q4 * 8 + 0]) * inv, __uint_as_float(r[q4 * 8 + 1]) * inv);
-                        v.y = pack_bf16x2(__uint_as_float(r[q4 * 8 + 2]) * inv, __uint_as_float(r[q4 * 8 + 3]) * inv);
-                        v.z = pack_bf16x2(__uint_as_float(r[q4 * 8 + 4]) * inv, __uint_as_float(r[q4 * 8 + 5]) * inv);
-                        v.w = pack_bf16x2(__uint_as_float(r[q4 * 8 + 6]) * inv, __uint_as_float(r[q4 * 8 + 7]) * inv);
-                        dst[c * 4 + q4] = v;
-                    }
+                for (int pc = 0; pc < 8; ++pc) {
+                    const uint32_t* x = &r[pc >> 2][(pc & 3) * 8];
+                    uint4 v;
+                    v.x = pack_bf16x2(__uint_as_float(x[0]) * inv, __uint_as_float(x[1]) * inv);
+                    v.y = pack_bf16x2(__uint_as_float(x[2]) * inv, __uint_as_float(x[3]) * inv);
+                    v.z = pack_bf16x2(__uint_as_float(x[4]) * inv, __uint_as_float(x[5]) * inv);
+                    v.w = pack_bf16x2(__uint_as_float(x[6]) * inv, __uint_as_float(x[7]) * inv);
+                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(stg + (uint32_t)(lane * 128 + ((pc ^ (lane & 7)) << 4))),
+                                 "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
                 }
+                __syncwarp();
+                if (tl_me && hh == 0) PA_TL(14 + t, (int)it, 1);
+                uint4 w[8];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int rr = 4 * i + (lane >> 3), pc = lane & 7;
+                    // volatile (ordered behind the stores and the warp barrier) but no memory clobber: the eight loads and
+                    // the global stores that consume them are scheduled freely
+                    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w[i].x), "=r"(w[i].y), "=r"(w[i].z), "=r"(w[i].w)
+                                 : "r"(stg + (uint32_t)(rr * 128 + ((pc ^ (rr & 7)) << 4))));
+                }
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int rr = 4 * i + (lane >> 3), pc = lane & 7;
+                    if ((vmask >> rr) & 1u)
+                        *reinterpret_cast<uint4*>(out0 + (int64_t)rr * p.Hq * D + hh * 64 + pc * 8) = w[i];
+                }
+                __syncwarp();
+                if (tl_me && hh == 0) PA_TL(14 + t, (int)it, 2);
             }
             tc_fence_before();
+            if (tl_me) PA_TL(12 + t, (int)it, 2);
         }
     }
 
