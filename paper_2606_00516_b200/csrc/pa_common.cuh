@@ -5,6 +5,20 @@
 #include <cuda.h>
 #include <cstdint>
 
+// (needs a PlanView named `pl` in scope)
+// Development instrumentation (-DPA_TIMELINE=<cta>): clock64 stamps of the hand-offs of one CTA, written into the
+// (otherwise idle) redo region of the workspace as int64 [role][step][4]; roles 0/1 = softmax groups, 2/3 = MMA warp
+// per q-head tile.  Not compiled into the product library.
+#ifdef PA_TIMELINE
+#define PA_TL(role, step, field)                                                                                   \
+    do {                                                                                                           \
+        if ((int)blockIdx.x == PA_TIMELINE && (step) < 400)                                                        \
+            reinterpret_cast<long long*>(pl.redo)[(((role) * 400) + (step)) * 4 + (field)] = clock64();            \
+    } while (0)
+#else
+#define PA_TL(role, step, field) do { } while (0)
+#endif
+
 namespace pa {
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {

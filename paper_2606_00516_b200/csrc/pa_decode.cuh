@@ -112,7 +112,7 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
     int4 d0 = make_int4(0, 0, -1, 0), d1 = d0;           // current bundle: {grp_begin, blk_begin, grp_end, blk_end}, parts
     int grp = 0, grp_last = -1;
     // A group of the walk, with its context length in flight: {seq, kv head, blk_begin, blk_end or -1}, {ctx, part_base, part}
-    auto next_group = [&](int4& ga, int4& gb) -> bool {
+    auto next_group = [&](int4& ga, int4& gb, int& gn) -> bool {
         while (grp > grp_last) {
             if (!have_next) return false;
             d0 = nd0; d1 = nd1;
@@ -134,29 +134,36 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
         const int seq = grp / p.Hkv, kvh = grp - seq * p.Hkv;
         const bool first = grp == d0.x, last = grp == d0.z;
         ga = make_int4(seq, kvh, first ? d0.y : 0, last ? d0.w : -1);
-        gb = make_int4(__ldg(p.context_lens + seq), first ? d1.x : (last ? d1.z : -1), first ? d1.y : (last ? d1.w : 1), 0);
+        // the ids of the group's first two blocks are requested together with its context length (their addresses do
+        // not depend on it; the second entry is inside the table row and never dereferenced unless the block exists)
+        const int32_t* bt0 = p.block_tables + (int64_t)seq * p.max_blocks_per_seq + ga.z;
+        gb = make_int4(__ldg(p.context_lens + seq), first ? d1.x : (last ? d1.z : -1), first ? d1.y : (last ? d1.w : 1), __ldg(bt0));
+        gn = (ga.z + 1 < p.max_blocks_per_seq) ? __ldg(bt0 + 1) : 0;
         ++grp;
         return true;
     };
     // turns a fetched group into the item descriptor (DecItem layout) once its context length has arrived
-    auto resolve = [&](int4& ga, int4& gb) {
+    auto resolve = [&](int4& ga, int4& gb, int& first_id) {
         const int kv_len = gb.x + 1, nblk = (kv_len + kBlock - 1) / kBlock;
         if (ga.w < 0) ga.w = nblk;
         const int part = gb.z;
+        first_id = gb.w;
         gb = make_int4(kv_len, gb.y, gb.y < 0 ? 0 : (part >> 16), gb.y < 0 ? 1 : (part & 0xffff));
     };
     // Two-deep software pipeline over items so that no load is waited on where it is issued:
-    //   stage 2: context length of item i+2 in flight;  stage 1: item i+1 resolved, its first block ids in flight.
+    //   stage 2: context length and first block ids of item i+2 in flight;  stage 1: item i+1 resolved.
     int4 a1 = make_int4(0, 0, 0, 0), b1 = a1, a2 = a1, b2 = a1;
-    int blkid1 = 0, blkid1n = 0;      // ids of the first two blocks of the stage-1 item
-    bool v2 = next_group(a2, b2);
+    int blkid1 = 0, blkid1n = 0, n2 = 0;      // ids of the first two blocks of the stage-1 item; second id of stage 2
+    if (threadIdx.x == 0) PA_TL(4, 0, 2);
+    bool v2 = next_group(a2, b2, n2);
     bool v1 = v2;
+    if (threadIdx.x == 0) PA_TL(4, 0, 3);
     if (v1) {
-        a1 = a2; b1 = b2;
-        resolve(a1, b1);
-        blkid1 = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z);
-        if (a1.z + 1 < a1.w) blkid1n = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z + 1);
-        v2 = next_group(a2, b2);
+        a1 = a2; b1 = b2; blkid1n = n2;
+        resolve(a1, b1, blkid1);
+        if (threadIdx.x == 0) PA_TL(4, 1, 0);
+        v2 = next_group(a2, b2, n2);
+        if (threadIdx.x == 0) PA_TL(4, 1, 1);
     }
     while (v1) {
         const int4 a = a1, b = b1;
@@ -164,11 +171,9 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
         // ---- advance the pipeline
         v1 = v2;
         if (v1) {
-            a1 = a2; b1 = b2;
-            resolve(a1, b1);
-            blkid1 = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z);
-            if (a1.z + 1 < a1.w) blkid1n = __ldg(p.block_tables + (int64_t)a1.x * p.max_blocks_per_seq + a1.z + 1);
-            v2 = next_group(a2, b2);
+            a1 = a2; b1 = b2; blkid1n = n2;
+            resolve(a1, b1, blkid1);
+            v2 = next_group(a2, b2, n2);
         }
         // ---- open the item: descriptor + Q rows into the fifo entry
         const int seq = a.x, kvh = a.y, blk_end = a.w, kv_len = b.x;
@@ -176,7 +181,9 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
         const int32_t* bt = p.block_tables + (int64_t)seq * p.max_blocks_per_seq;
         {
             const uint32_t fs = i_iss % FQ;
+            if (threadIdx.x == 0) PA_TL(1, (int)i_iss, 0);
             mbar_wait(bar + Cfg::kOffFEmpty + 8 * fs, ((i_iss / FQ) & 1u) ^ 1u);
+            if (threadIdx.x == 0) PA_TL(1, (int)i_iss, 1);
             const uint32_t d = smem_u32(aux + Cfg::kOffDesc + 32 * fs);
             asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(d), "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w) : "memory");
             asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(d + 16), "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w) : "memory");
@@ -187,6 +194,7 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
 #pragma unroll
             for (int c = 0; c < D / 64; ++c) tma_load_2d(q_u32 + fs * Cfg::kQSlot + c * 1024, tmQd, ff, c * 64, qrow);
             ++i_iss;
+            if (threadIdx.x == 0) PA_TL(1, (int)i_iss - 1, 2);
         }
         // ---- stream the K and V tiles of the item's blocks
         while (blk < blk_end) {
@@ -225,6 +233,7 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
                 }
             }
         }
+        if (threadIdx.x == 0) PA_TL(1, (int)i_iss - 1, 3);
     }
     // ---- sentinel item: tells the consumer that the stream is finished
     {
@@ -320,6 +329,19 @@ __device__ __forceinline__ void decode_merge(const AttnParams& p, const DecItem&
     }
 }
 
+// The filled rows of a partly filled last block are fetched (8/4/2/1-row boxes); the other rows of the V slot keep
+// whatever the slot held.  P of those rows is exactly 0, but 0 x NaN would poison O, so they are cleared: the slot is
+// [plane][row][128 B] = 256 consecutive 16-byte chunks, lane l owns chunks l + 32k (row = (l / 8 + 4k) mod 16).
+__device__ __forceinline__ void decode_zero_dead_rows(uint32_t tile, int nvalid, int lane) {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int row = ((lane >> 3) + 4 * k) & 15;
+        if (row >= nvalid)
+            asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(tile + (uint32_t)(lane + 32 * k) * 16u), "r"(0u) : "memory");
+    }
+    __syncwarp();
+}
+
 // ------------------------------------------------------------------------------------------------
 // Consumer warp of one stream.
 // ------------------------------------------------------------------------------------------------
@@ -338,7 +360,9 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
     uint32_t u_con = 0, i_con = 0;
     for (;;) {
         const uint32_t fs = i_con % FQ;
+        if (threadIdx.x == 128) PA_TL(0, (int)i_con, 0);
         mbar_wait(bar + Cfg::kOffFFull + 8 * fs, (i_con / FQ) & 1u);
+        if (threadIdx.x == 128) PA_TL(0, (int)i_con, 1);
         const DecItem ci = *reinterpret_cast<const DecItem*>(aux + Cfg::kOffDesc + 32 * fs);
         if (ci.seq < 0) break;
         const uint32_t qs = q_u32 + fs * Cfg::kQSlot;
@@ -348,7 +372,98 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
 #pragma unroll
         for (int i = 0; i < KS; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
 
-        for (int blk = ci.blk_begin; blk < ci.blk_end; ++blk) {
+        int blk = ci.blk_begin;
+        if constexpr (H == 1) {
+            // ---- two blocks per iteration (D = 128: K, V, K, V of the pair fit the ring).  Both score tiles are computed
+            // first, ONE online-softmax update serves the 32 tokens (half the shuffles, exponentials of the correction
+            // and rescale multiplies per block), then both PV products: a lone in-order warp hides the latencies of the
+            // four MMA chains in each other.  Only the second block of a pair can be a partly filled last block.
+            for (; blk + 1 < ci.blk_end; blk += 2) {
+                const int nvalidB = min(16, ci.kv_len - (blk + 1) * kBlock);
+                const uint32_t sKA = u_con % R, sVA = (u_con + 1) % R, sKB = (u_con + 2) % R, sVB = (u_con + 3) % R;
+                const uint32_t phKA = (u_con / R) & 1u, phVA = ((u_con + 1) / R) & 1u, phKB = ((u_con + 2) / R) & 1u,
+                               phVB = ((u_con + 3) / R) & 1u;
+                float sA0[4] = {0.f, 0.f, 0.f, 0.f}, sA1[4] = {0.f, 0.f, 0.f, 0.f};
+                float sB0[4] = {0.f, 0.f, 0.f, 0.f}, sB1[4] = {0.f, 0.f, 0.f, 0.f};
+                const uint32_t tKA = ring_u32 + sKA * Cfg::kUnit, tKB = ring_u32 + sKB * Cfg::kUnit;
+                const uint32_t rowk = r8 + 8 * (mi & 1);
+                mbar_wait(bar + 8 * sKA, phKA);
+                mbar_wait(bar + 8 * sKB, phKB);
+                if (threadIdx.x == 128) PA_TL(2, (int)i_con, 0);
+#pragma unroll
+                for (int k2 = 0; k2 < 4; ++k2) {
+                    uint32_t qf[4];
+                    const uint32_t cq = 4 * k2 + mi;
+                    ldmatrix_x4(qf, qs + (cq >> 3) * 1024 + swz128(r8, cq & 7));
+#pragma unroll
+                    for (int kk = 0; kk < 2; ++kk) {
+                        const uint32_t chunk = 2 * (2 * k2 + kk) + (mi >> 1);
+                        const uint32_t off = (chunk >> 3) * 2048 + swz128(rowk, chunk & 7);
+                        uint32_t a[4], b[4];
+                        ldmatrix_x4(a, tKA + off);
+                        ldmatrix_x4(b, tKB + off);
+                        if (kk) { mma_bf16_16816(sA1, a, qf[2], qf[3]); mma_bf16_16816(sB1, b, qf[2], qf[3]); }
+                        else    { mma_bf16_16816(sA0, a, qf[0], qf[1]); mma_bf16_16816(sB0, b, qf[0], qf[1]); }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) { mbar_arrive(bar + Cfg::kOffEmpty + 8 * sKA); mbar_arrive(bar + Cfg::kOffEmpty + 8 * sKB); }
+                if (threadIdx.x == 128) PA_TL(2, (int)i_con, 1);
+                // tokens g, g + 8 of block A (s0..s3) and of block B (s4..s7), heads 2t / 2t + 1
+                float s0 = (sA0[0] + sA1[0]) * p.scale_log2, s1 = (sA0[1] + sA1[1]) * p.scale_log2;
+                float s2 = (sA0[2] + sA1[2]) * p.scale_log2, s3 = (sA0[3] + sA1[3]) * p.scale_log2;
+                float s4 = (sB0[0] + sB1[0]) * p.scale_log2, s5 = (sB0[1] + sB1[1]) * p.scale_log2;
+                float s6 = (sB0[2] + sB1[2]) * p.scale_log2, s7 = (sB0[3] + sB1[3]) * p.scale_log2;
+                if (g >= nvalidB) { s4 = -INFINITY; s5 = -INFINITY; }
+                if (g + 8 >= nvalidB) { s6 = -INFINITY; s7 = -INFINITY; }
+                float mx0 = fmaxf(fmaxf(s0, s2), fmaxf(s4, s6)), mx1 = fmaxf(fmaxf(s1, s3), fmaxf(s5, s7));
+#pragma unroll
+                for (int off = 4; off <= 16; off <<= 1) {
+                    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, off));
+                    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, off));
+                }
+                const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
+                const float c0 = fast_exp2(m0 - mn0), c1 = fast_exp2(m1 - mn1);
+                const float p0 = fast_exp2(s0 - mn0), p1 = fast_exp2(s1 - mn1), p2 = fast_exp2(s2 - mn0), p3 = fast_exp2(s3 - mn1);
+                const float p4 = fast_exp2(s4 - mn0), p5 = fast_exp2(s5 - mn1), p6 = fast_exp2(s6 - mn0), p7 = fast_exp2(s7 - mn1);
+                m0 = mn0; m1 = mn1;
+                l0 = l0 * c0 + (p0 + p2) + (p4 + p6);
+                l1 = l1 * c1 + (p1 + p3) + (p5 + p7);
+                if (__any_sync(0xffffffffu, c0 != 1.f || c1 != 1.f)) {     // the running max of long contexts rarely moves
+#pragma unroll
+                    for (int i = 0; i < KS; ++i) { o[i][0] *= c0; o[i][1] *= c1; o[i][2] *= c0; o[i][3] *= c1; }
+                }
+                const uint32_t pA0 = movmatrix_trans(pack_bf16x2(p0, p1)), pA1 = movmatrix_trans(pack_bf16x2(p2, p3));
+                const uint32_t pB0 = movmatrix_trans(pack_bf16x2(p4, p5)), pB1 = movmatrix_trans(pack_bf16x2(p6, p7));
+                const uint32_t tVA = ring_u32 + sVA * Cfg::kUnit, tVB = ring_u32 + sVB * Cfg::kUnit;
+                const uint32_t rowv = r8 + 8 * (mi >> 1);
+                if (threadIdx.x == 128) PA_TL(2, (int)i_con, 2);
+                mbar_wait(bar + 8 * sVA, phVA);
+                mbar_wait(bar + 8 * sVB, phVB);
+                if (threadIdx.x == 128) PA_TL(2, (int)i_con, 3);
+                if (nvalidB < 16) decode_zero_dead_rows(tVB, nvalidB, lane);
+                if (threadIdx.x == 128) PA_TL(3, (int)i_con, 0);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {      // block A first, then block B: dependent MMAs of o[i] are eight apart
+                    const uint32_t chunk = 2 * i + (mi & 1);
+                    uint32_t a[4];
+                    ldmatrix_x4_trans(a, tVA + (chunk >> 3) * 2048 + swz128(rowv, chunk & 7));
+                    mma_bf16_16816(o[i], a, pA0, pA1);
+                }
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const uint32_t chunk = 2 * i + (mi & 1);
+                    uint32_t b[4];
+                    ldmatrix_x4_trans(b, tVB + (chunk >> 3) * 2048 + swz128(rowv, chunk & 7));
+                    mma_bf16_16816(o[i], b, pB0, pB1);
+                }
+                if (nvalidB < 16) fence_proxy_async();   // generic-proxy zero fill before the slot's next TMA write
+                __syncwarp();
+                if (lane == 0) { mbar_arrive(bar + Cfg::kOffEmpty + 8 * sVA); mbar_arrive(bar + Cfg::kOffEmpty + 8 * sVB); }
+                u_con += 4;
+            }
+        }
+        for (; blk < ci.blk_end; ++blk) {
             const int nvalid = min(16, ci.kv_len - blk * kBlock);
             // ---- S^T[16 tok x 8 heads] = K[16 x D] · Q^T[D x 8]
             float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb[4] = {0.f, 0.f, 0.f, 0.f};
@@ -407,14 +522,7 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
                 const uint32_t slot = u_con % R;
                 mbar_wait(bar + 8 * slot, (u_con / R) & 1u);
                 const uint32_t tile = ring_u32 + slot * Cfg::kUnit;
-                if (nvalid < 16) {   // last, partly filled block: unused V rows may hold anything (NaN): zero them
-                    const int nz = (16 - nvalid) * 8;                    // 16-byte chunks per 64-column box
-#pragma unroll
-                    for (int qd = 0; qd < 2; ++qd)
-                        for (int idx = lane; idx < nz; idx += 32)
-                            asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(tile + qd * 2048 + nvalid * 128 + idx * 16), "r"(0u) : "memory");
-                    __syncwarp();
-                }
+                if (nvalid < 16) decode_zero_dead_rows(tile, nvalid, lane);
                 const uint32_t row = r8 + 8 * (mi >> 1);               // token
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
@@ -430,8 +538,7 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
             }
         }
         // ---------------- item finished
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar + Cfg::kOffFEmpty + 8 * fs);    // Q rows and descriptor are no longer needed
+        if (threadIdx.x == 128) PA_TL(0, (int)i_con, 2);
         ++i_con;
 #pragma unroll
         for (int off = 4; off <= 16; off <<= 1) {
@@ -440,16 +547,36 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
         }
         const int ha = 2 * t, hb = 2 * t + 1;
         if (ci.n_parts == 1) {
-            // O^T fragments -> (head = g, d = 16i + 2t, +1) via movmatrix: 4-byte stores, 16 B contiguous per head
+            // O^T fragments (row d, columns head 2t / 2t+1) -> out[q_row][h0 .. h0+G)[:], G·D·2 contiguous bytes: the 8x8
+            // matrices are stored TRANSPOSED (stmatrix.trans) into the item's (now idle) Q slot as [head][d] rows, 16-byte
+            // chunks XOR-swizzled by head, and leave as whole 16-byte vectors, consecutive lanes on consecutive addresses
             const float i0 = 1.f / l0, i1 = 1.f / l1;
-            uint32_t* dst = reinterpret_cast<uint32_t*>(p.out + ((int64_t)q_row * p.Hq + h0 + g) * D) + t;
+            __syncwarp();                                   // every lane is done with the Q rows of the slot
 #pragma unroll
-            for (int i = 0; i < KS; ++i) {
-                const uint32_t y0 = movmatrix_trans(pack_bf16x2(o[i][0] * i0, o[i][1] * i1));
-                const uint32_t y1 = movmatrix_trans(pack_bf16x2(o[i][2] * i0, o[i][3] * i1));
-                if (g < G) { dst[8 * i] = y0; dst[8 * i + 4] = y1; }
+            for (int i = 0; i < KS; i += 2) {
+                const uint32_t mm = (uint32_t)lane >> 3, hh = (uint32_t)lane & 7u;     // matrix (i + mm/2, half mm%2), head row hh
+                const uint32_t cc = (uint32_t)(2 * (i + (int)(mm >> 1))) + (mm & 1u);  // 16-byte chunk = 8 consecutive d
+                const uint32_t addr = qs + hh * (uint32_t)(2 * D) + (((cc ^ hh) & (uint32_t)(D / 8 - 1))) * 16u;
+                asm volatile("stmatrix.sync.aligned.m8n8.x4.trans.shared.b16 [%0], {%1, %2, %3, %4};"
+                             ::"r"(addr), "r"(pack_bf16x2(o[i][0] * i0, o[i][1] * i1)), "r"(pack_bf16x2(o[i][2] * i0, o[i][3] * i1)),
+                               "r"(pack_bf16x2(o[i + 1][0] * i0, o[i + 1][1] * i1)), "r"(pack_bf16x2(o[i + 1][2] * i0, o[i + 1][3] * i1))
+                             : "memory");
             }
+            __syncwarp();
+            uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)q_row * p.Hq + h0) * D);
+            for (int q = lane; q < G * (D / 8); q += 32) {
+                const uint32_t hh = (uint32_t)q / (uint32_t)(D / 8), cc = (uint32_t)q % (uint32_t)(D / 8);
+                uint4 v;
+                asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                             : "r"(qs + hh * (uint32_t)(2 * D) + ((cc ^ hh) & (uint32_t)(D / 8 - 1)) * 16u));
+                dst[q] = v;
+            }
+            __syncwarp();
+            fence_proxy_async();                            // generic-proxy writes before the slot's next TMA fill
+            if (lane == 0) mbar_arrive(bar + Cfg::kOffFEmpty + 8 * fs);    // Q slot and descriptor may be refilled
         } else {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar + Cfg::kOffFEmpty + 8 * fs);    // Q rows and descriptor are no longer needed
             const int ps = ci.part_base + ci.part_idx;
             if (g == 0) {
                 if (ha < G) pl.part_ml[ps * kMaxGroup + ha] = make_float2(m0, l0);
@@ -476,6 +603,7 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
                 if (lane == 0) *ctr = 0;                      // self-reset for the next launch
             }
         }
+        if (threadIdx.x == 128) PA_TL(0, (int)i_con - 1, 3);
     }
 }
 
@@ -488,6 +616,7 @@ __device__ __forceinline__ void decode_role(const AttnParams& p, const CUtensorM
                                             int dec_rank) {
     using Cfg = DecodeCfg<D>;
     const int warp = threadIdx.x >> 5, lane = lane_id();
+    [[maybe_unused]] const PlanView& pl = p.plan;
     if (warp < kDecodeProducerWarps) {
         if (lane < kStreamsPerProducer) {
             const int s = warp * kStreamsPerProducer + lane;

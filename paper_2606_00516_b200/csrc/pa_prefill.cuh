@@ -98,19 +98,6 @@ __device__ __forceinline__ void prefill_init_barriers(PrefillCtrl* c, int nq) { 
     mbar_arrive(smem_u32(&c->turn[0]));       // tile 0 goes first
 }
 
-// Development instrumentation (-DPA_TIMELINE=<cta>): clock64 stamps of the hand-offs of one CTA, written into the
-// (otherwise idle) redo region of the workspace as int64 [role][step][4]; roles 0/1 = softmax groups, 2/3 = MMA warp
-// per q-head tile.  Not compiled into the product library.
-#ifdef PA_TIMELINE
-#define PA_TL(role, step, field)                                                                                   \
-    do {                                                                                                           \
-        if ((int)blockIdx.x == PA_TIMELINE && (step) < 400)                                                        \
-            reinterpret_cast<long long*>(pl.redo)[(((role) * 400) + (step)) * 4 + (field)] = clock64();            \
-    } while (0)
-#else
-#define PA_TL(role, step, field) do { } while (0)
-#endif
-
 // exp2 of two finite floats on the FMA / integer pipes: x = n + f with n = round(x), f in [-0.5, 0.5];
 // 2^f by a cubic (near-minimax, relative error 7.5e-5: below the bf16 rounding of P by a factor of 25), 2^n by adding
 // n to the exponent field.  x is clamped at -126 (result 2^-126, which rounds P to ~1e-38: nothing in fp32 sums).
