@@ -398,6 +398,61 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                     asm volatile("" : "+l"(dbv), "+l"(dbk));                        // materialised here, behind the S burst
                 }
                 j = 2 * n_fast;
+            } else {
+                // ---- steady state for one-step K/V tiles (D = 256: KT = HT = 64): two steps per iteration so that the
+                // score buffer is a compile-time constant; per step PV(j) on V tile j, then S(j + 2) on K tile j + 2.
+                const int n_fast = active ? max(0, (nstep_u - 3) / 2) : 0;      // pairs (2i, 2i + 1) with 2i + 3 <= nstep_u - 2
+                uint32_t ek = ring0 + 4, ev = ring0 + 1;               // ring entries: K tile j + 2, V tile j
+                uint32_t kst = ek % ST, kph = (ek / ST) & 1u, vst = ev % ST, vph = (ev / ST) & 1u;
+                auto desc_v = [&](uint32_t st) { return umma_desc_sw128(sbase + Cfg::kOffRing + st * Cfg::kStageBytes, KT * 128, 1024); };
+                auto desc_k = [&](uint32_t st) { return umma_desc_sw128(sbase + Cfg::kOffRing + st * Cfg::kStageBytes, 16, 1024); };
+                uint64_t dbv = desc_v(vst), dbk = desc_k(kst);
+                uint64_t dp[2] = {0, 0};
+                if constexpr (!kPinTmem) {
+                    dp[0] = umma_desc_sw128(sbase + Cfg::kOffP + (2 * t) * Cfg::kPBytes, 16, 1024);
+                    dp[1] = umma_desc_sw128(sbase + Cfg::kOffP + (2 * t + 1) * Cfg::kPBytes, 16, 1024);
+                }
+                if (n_fast > 0) mbar_wait(smem_u32(&ctrl->kv_full[vst]), vph);       // V tile 0
+                for (int i = 0; i < n_fast; ++i) {
+#pragma unroll
+                    for (int b = 0; b < 2; ++b) {
+                        mbar_wait(smem_u32(&ctrl->p_full[t][b]), (pph >> b) & 1u);
+                        tc_fence_after();
+                        if (elect_one()) {
+#pragma unroll
+                            for (int ks = 0; ks < HT / kBlock; ++ks) {
+                                const uint64_t db = dbv + (uint64_t)(ks * (2048 >> 4));
+                                const uint32_t acc = (i > 0 || b > 0 || ks > 0) ? 1u : 0u;
+                                if constexpr (kPinTmem) umma_ts(ocol, scol0 + b * HT + ks * 8, db, idescO, acc);
+                                else umma_ss(ocol, dp[b] + (uint64_t)((ks * 32) >> 4), db, idescO, acc);
+                            }
+                            umma_commit(smem_u32(&ctrl->pv_done[t]));
+                            umma_commit(smem_u32(&ctrl->kv_empty[vst]));
+                        }
+                        __syncwarp();
+                        mbar_wait(smem_u32(&ctrl->kv_full[kst]), kph);               // K tile j + 2
+                        tc_fence_after();
+                        if (elect_one()) {
+#pragma unroll
+                            for (int ks = 0; ks < D / 16; ++ks) {
+                                const uint32_t oa = (uint32_t)(((ks >> 2) * (kQTile * 128) + (ks & 3) * 32) >> 4);
+                                const uint32_t ob = (uint32_t)(((ks >> 2) * (KT * 128) + (ks & 3) * 32) >> 4);
+                                umma_ss(scol0 + b * HT, dq + oa, dbk + ob, idescS, ks > 0);
+                            }
+                            umma_commit(smem_u32(&ctrl->s_full[t][b]));
+                            umma_commit(smem_u32(&ctrl->kv_empty[kst]));
+                        }
+                        __syncwarp();
+                        kst += 2; if (kst >= ST) { kst -= ST; kph ^= 1u; }
+                        vst += 2; if (vst >= ST) { vst -= ST; vph ^= 1u; }
+                        mbar_wait(smem_u32(&ctrl->kv_full[vst]), vph);               // V tile j + 1 (it exists: >= 3 steps follow)
+                        dbv = desc_v(vst);
+                        dbk = desc_k(kst);
+                        asm volatile("" : "+l"(dbv), "+l"(dbk));
+                    }
+                    pph ^= 0x3u;
+                }
+                j = 2 * n_fast;
             }
             for (; j < nstep_u; ++j) {
                 const int i = j / HPT, hf = j % HPT, b = j & 1;
@@ -554,8 +609,10 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                 // ---- P = exp2(s*sl - m_ref*sl) -> bf16 (TMEM over S, or swizzled shared memory) and the step max,
                 // one pass, packed f32x2 math; the TMEM load of chunk c+1 is in flight while chunk c is processed.
                 const uint64_t sl2 = pack_f2(sl, sl), neg2 = pack_f2(neg, neg);
-                uint64_t lsum = pack_f2(0.f, 0.f);
-                float mx = NEG_INF;
+                // four row-sum and two max accumulators: a lone in-order warp would otherwise wait out the latency of a
+                // 32-deep dependent FADD2 / FMNMX3 chain
+                uint64_t lsum4[4] = {pack_f2(0.f, 0.f), pack_f2(0.f, 0.f), pack_f2(0.f, 0.f), pack_f2(0.f, 0.f)};
+                float mx2[2] = {NEG_INF, NEG_INF};
                 // Two copies of the pass: only the steps that straddle the diagonal pay for the mask (as one predicated
                 // pass the compare + select pair of every element ran on every step: a third of all instructions).
                 const int rel = limit - kbase;          // columns 0 .. rel of this step are visible to this row
@@ -577,7 +634,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                                 if (c * 32 + i > rel) s0 = NEG_INF;
                                 if (c * 32 + i + 1 > rel) s1 = NEG_INF;
                             }
-                            mx = fmaxf(mx, fmaxf(s0, s1));
+                            mx2[(i >> 1) & 1] = fmaxf(mx2[(i >> 1) & 1], fmaxf(s0, s1));
                             const uint64_t x = ffma2(pack_f2(s0, s1), sl2, neg2);
                             float x0, x1, p0, p1;
                             unpack_f2(x, x0, x1);
@@ -589,7 +646,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                                 p0 = fast_exp2(x0);
                                 p1 = fast_exp2(x1);
                             }
-                            lsum = fadd2(lsum, pack_f2(p0, p1));
+                            lsum4[(i >> 1) & 3] = fadd2(lsum4[(i >> 1) & 3], pack_f2(p0, p1));
                             pk[i >> 1] = pack_bf16x2(p0, p1);
                         }
                         if constexpr (kPinTmem) {
@@ -609,9 +666,10 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                 };
                 if (need_mask) pass(std::true_type{});
                 else pass(std::false_type{});
+                const float mx = fmaxf(mx2[0], mx2[1]);
                 {
                     float la, lb;
-                    unpack_f2(lsum, la, lb);
+                    unpack_f2(fadd2(fadd2(lsum4[0], lsum4[1]), fadd2(lsum4[2], lsum4[3])), la, lb);
                     l += la + lb;
                 }
                 m_run = fmaxf(m_run, mx);
