@@ -186,7 +186,8 @@ int32_t pa_crossover_eq7(const double* in, double* out);
  *        6 CTAs given the prefill role in the mixed launch, 7 decode bundles per stream (effective),
  *        8 prefill variant (0 P in TMEM, 1 P in shared memory, 2 plain kernel),
  *        9 host nanoseconds the last pa_plan call took (validation + lists + enqueue of the upload),
- *        10 pieces a decode bundle is handed out in (guided hand-out; 1 = whole bundles). */
+ *        10 pieces a decode bundle is handed out in (guided hand-out; 1 = whole bundles),
+ *        11 / 12 nanoseconds of (9) spent validating the descriptor / building the tile and bundle lists. */
 int64_t pa_plan_info(const pa_ctx* ctx, int32_t which);
 
 /* Library-owned message of the last error on ctx (valid until the next call on ctx); "" if none. */

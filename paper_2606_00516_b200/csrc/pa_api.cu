@@ -36,7 +36,7 @@ struct pa_ctx {
     PlanView view{};
     int32_t decode_ctas = 0, n_simple_tiles = 0, launches_per_call = 0, prefill_ctas = 0, p_in_tmem = 1;
     int32_t planned_n_tok = 0, n_items = 0, bundles_per_stream = 0, prefill_mode = 0, n_levels = 1;
-    int64_t plan_host_ns = 0;
+    int64_t plan_host_ns = 0, plan_ns_validate = 0, plan_ns_lists = 0;   // whole call; validation; tiles + bundles (rest: enqueue of the upload)
     // tensor-map cache
     const void* tm_k_ptr = nullptr;
     const void* tm_v_ptr = nullptr;
@@ -367,6 +367,7 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     const int32_t n_tok = n_seq > 0 ? h_cu[n_seq] : 0;
     if (n_tok > c.max_tokens) return fail(ctx, PA_ERR_INVALID, "pa_plan: n_tok > max_tokens");
     if (int32_t rc = check_device(ctx, "pa_plan")) return rc;
+    const auto t_valid = std::chrono::steady_clock::now();
 
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     const int stage = ctx->stage_next;
@@ -514,6 +515,7 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     const int32_t n_bundles = bc.n_bundles;
     const int64_t used = off_b + align_up((int64_t)n_bundles * sizeof(DecBundle), 256);
 
+    const auto t_lists = std::chrono::steady_clock::now();
     // ---- upload
     uint8_t* ws = static_cast<uint8_t*>(d_workspace);
     cudaError_t e = cudaMemsetAsync(ws + ctx->off_counters, 0, (size_t)(ctx->off_plan - ctx->off_counters), stream);
@@ -561,6 +563,8 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     ctx->launches_per_call = (dec_ctas + pre_ctas > 0) + (ctx->n_simple_tiles > 0);
     ctx->planned = true;
     ctx->plan_host_ns = std::chrono::duration_cast<std::chrono::nanoseconds>(std::chrono::steady_clock::now() - t_begin).count();
+    ctx->plan_ns_validate = std::chrono::duration_cast<std::chrono::nanoseconds>(t_valid - t_begin).count();
+    ctx->plan_ns_lists = std::chrono::duration_cast<std::chrono::nanoseconds>(t_lists - t_valid).count();
     return PA_OK;
 }
 
@@ -632,6 +636,8 @@ int64_t pa_plan_info(const pa_ctx* ctx, int32_t which) {
         case 8: return ctx->prefill_mode;
         case 9: return ctx->plan_host_ns;
         case 10: return ctx->n_levels;
+        case 11: return ctx->plan_ns_validate;
+        case 12: return ctx->plan_ns_lists;
 #ifdef PA_TIMELINE
         case 100: return ctx->off_redo;     // development instrumentation (pa_prefill.cuh PA_TL)
 #endif

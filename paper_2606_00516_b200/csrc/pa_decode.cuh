@@ -108,7 +108,10 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
         const int bb = ticket_bundle(b_next, lvl_next);
         nd0 = __ldg(bundles + 2 * bb); nd1 = __ldg(bundles + 2 * bb + 1);
     }
-    int b_after = have_next ? p.decode_workers + atomicAdd(&pl.queue[0], 1) : n_tickets;
+    // no ticket beyond the statically assigned ones (pure decode with one bundle per stream): no queue traffic at all —
+    // 1184 lanes hitting one counter at kernel start cost the first item ~1.5 us
+    const bool dynamic = n_tickets > p.decode_workers;
+    int b_after = (have_next && dynamic) ? p.decode_workers + atomicAdd(&pl.queue[0], 1) : n_tickets;
     int4 d0 = make_int4(0, 0, -1, 0), d1 = d0;           // current bundle: {grp_begin, blk_begin, grp_end, blk_end}, parts
     int grp = 0, grp_last = -1;
     // A group of the walk, with its context length in flight: {seq, kv head, blk_begin, blk_end or -1}, {ctx, part_base, part}
