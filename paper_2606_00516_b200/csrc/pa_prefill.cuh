@@ -309,9 +309,6 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
             const bool active = t < nact_u, both = nact_u == NQ;
             mbar_wait(smem_u32(&ctrl->q_full), it & 1u);
             tc_fence_after();
-#ifdef PA_STAGGER_NS
-            if (t == 1) __nanosleep(PA_STAGGER_NS);
-#endif
             for (int js = 0; js < min(2, nstep_u); ++js) step_S(js, active, nstep_u);
             int j = 0;
             if constexpr (HPT == 2) {
