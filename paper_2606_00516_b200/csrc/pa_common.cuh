@@ -15,8 +15,16 @@
         if ((int)blockIdx.x == PA_TIMELINE && (step) < 400)                                                        \
             reinterpret_cast<long long*>(pl.redo)[(((role) * 400) + (step)) * 4 + (field)] = clock64();            \
     } while (0)
+// per-CTA %globaltimer stamps (all CTAs): int64 [cta][4] behind the per-role stamps
+#define PA_TL_CTA(field)                                                                                           \
+    do {                                                                                                           \
+        unsigned long long gt_;                                                                                    \
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_));                                                    \
+        reinterpret_cast<unsigned long long*>(pl.redo)[16 * 400 * 4 + blockIdx.x * 4 + (field)] = gt_;             \
+    } while (0)
 #else
 #define PA_TL(role, step, field) do { } while (0)
+#define PA_TL_CTA(field) do { } while (0)
 #endif
 
 namespace pa {

@@ -555,6 +555,7 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
             // chunks XOR-swizzled by head, and leave as whole 16-byte vectors, consecutive lanes on consecutive addresses
             const float i0 = 1.f / l0, i1 = 1.f / l1;
             __syncwarp();                                   // every lane is done with the Q rows of the slot
+            if (threadIdx.x == 128) PA_TL(5, (int)i_con - 1, 0);
 #pragma unroll
             for (int i = 0; i < KS; i += 2) {
                 const uint32_t mm = (uint32_t)lane >> 3, hh = (uint32_t)lane & 7u;     // matrix (i + mm/2, half mm%2), head row hh
@@ -566,6 +567,7 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
                              : "memory");
             }
             __syncwarp();
+            if (threadIdx.x == 128) PA_TL(5, (int)i_con - 1, 1);
             uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)q_row * p.Hq + h0) * D);
             for (int q = lane; q < G * (D / 8); q += 32) {
                 const uint32_t hh = (uint32_t)q / (uint32_t)(D / 8), cc = (uint32_t)q % (uint32_t)(D / 8);
@@ -575,7 +577,9 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
                 dst[q] = v;
             }
             __syncwarp();
+            if (threadIdx.x == 128) PA_TL(5, (int)i_con - 1, 2);
             fence_proxy_async();                            // generic-proxy writes before the slot's next TMA fill
+            if (threadIdx.x == 128) PA_TL(5, (int)i_con - 1, 3);
             if (lane == 0) mbar_arrive(bar + Cfg::kOffFEmpty + 8 * fs);    // Q slot and descriptor may be refilled
         } else {
             __syncwarp();

@@ -137,7 +137,7 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
     PrefillCtrl* ctrl = reinterpret_cast<PrefillCtrl*>(tiles + kTileRegion);
     uint8_t* dec_aux = tiles + kTileRegion + kCtrlBytes;
     const PlanView& pl = p.plan;
-    if (threadIdx.x == 0) PA_TL(15, 399, 0);
+    if (threadIdx.x == 0) { PA_TL(15, 399, 0); PA_TL_CTA(0); }
     // set-up spread over threads (it is on the critical path of microsecond-scale launches): thread 0 the prefill
     // barriers, threads 32.. one decode stream each, thread 64 the descriptor prefetches
     if (threadIdx.x == 0 && pl.n_units > 0) prefill_init_barriers(ctrl, PrefillCfg<D, kPinTmem>::NQ);
@@ -176,7 +176,7 @@ pa_attention_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tmQ,
                 decode_role<D>(p, &tmQd, &tmK, &tmV, &tails, tiles, dec_aux, starts_prefill ? -1 : dec_rank);
         }
         __syncthreads();
-        if (threadIdx.x == 0) PA_TL(15, 397 + pass, 0);
+        if (threadIdx.x == 0) { PA_TL(15, 397 + pass, 0); PA_TL_CTA(1 + pass); }
     }
     // The last CTA to leave resets the queues for the next launch and recomputes, with the plain row loop, the prefill
     // rows whose one-pass softmax overflowed (normally none).  Pattern: writers fence before the counting atomic,
