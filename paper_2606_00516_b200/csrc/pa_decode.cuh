@@ -274,7 +274,10 @@ __device__ __forceinline__ void decode_merge(const AttnParams& p, const DecItem&
         for (int k = 0; k < VPL; ++k) acc[h][k] = 0.f;
     // PB parts' partial outputs are fetched together (as many as the register budget allows) and the (m, l) of
     // the next four parts are already in flight, so a group of n parts costs ~n/PB + n/4 L2 round trips
-    constexpr int PB = (GG * VPL <= 16) ? 2 : 1;     // inlined in the consumer: keep within its register budget
+    // the accumulators of the item are dead by now, so 64 registers can hold partial outputs in flight:
+    // a group of many parts (a few long sequences split over every stream) is merged by ONE warp at the very end of the
+    // launch, and its time is the number of L2 round trips
+    constexpr int PB = (GG * VPL <= 16) ? 4 : ((GG * VPL <= 32) ? 2 : 1);
     float2 ml_next = make_float2(-INFINITY, 0.f);
     if (pi < np) ml_next = __ldcg(ml_base + pi * kMaxGroup + hl);
     for (int c0 = 0; c0 < np; c0 += 4) {
