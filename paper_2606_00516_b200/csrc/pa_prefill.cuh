@@ -544,6 +544,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
             // that one step, which floating point absorbs (P <= 2^64 is left alone; beyond it the row is fixed up
             // exactly, see below).
             float m_ref = NEG_INF, m_run = NEG_INF, l = 0.f;
+            bool grew = false;
             // O_t may be touched only when every PV issued so far has completed.  PV(j-1) is the last one issued when
             // step j is being processed (PV(j) needs this step's P), and PV(j-2) has completed (s_full of step j was
             // committed behind it), so the commit count of pv_done is pv_base + j - 1 or pv_base + j: waiting for the
@@ -594,7 +595,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                         }
                     }
                     m_ref = m_run = mx;
-                } else if (__any_sync(0xffffffffu, (m_run - m_ref) * sl > 8.f)) {
+                } else if (grew) {
                     // lazy correction of the O row and l
                     const float alpha = fast_exp2((m_ref - m_run) * sl);
                     l *= alpha;
@@ -670,7 +671,10 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                     l += la + lb;
                 }
                 m_run = fmaxf(m_run, mx);
-                if (j > 0 && __any_sync(0xffffffffu, (mx - m_ref) * sl > 64.f)) {
+                // one vote per step: did any row's running max outgrow its reference by more than 2^8?  (the next step then
+                // moves the reference; a step that outgrew it by more than 2^64 is a subset and fixed up right here)
+                grew = __any_sync(0xffffffffu, (m_run - m_ref) * sl > 8.f);
+                if (grew && j > 0 && __any_sync(0xffffffffu, (mx - m_ref) * sl > 64.f)) {
                     // rare: this step outgrew the reference by more than 2^64.  Its P (finite up to 2^127) is scaled
                     // down by the exact power of two alpha, together with l and the O row, and the reference moves.
                     const bool mine = (mx - m_ref) * sl > 64.f;
@@ -700,6 +704,7 @@ __device__ void prefill_role(const AttnParams& p, const CUtensorMap* tmQ, const 
                     }
                     wait_pv(j);
                     rescale_o(alpha);
+                    grew = __any_sync(0xffffffffu, (m_run - m_ref) * sl > 8.f);
                 }
                 if (tl_me) PA_TL(t, tl_step, 2);
                 if (lane == 0) PA_TL(4 + warp, tl_step, 2);
