@@ -7,7 +7,7 @@
 // Design.  One work unit = (128-row query tile of one chunk, KV head, group of NQ q heads
 // that share that KV head).  The NQ q-head tiles of a unit stream the SAME K/V tiles (GQA: K/V are read
 // once per KV head, not once per q head).  The keys are processed in steps of HT = 64; the scores of a
-// q-head tile live in TWO TMEM buffers (step j in buffer j & 1), so the MMA warp computes S(j+1) and S(j+2)
+// q-head tile live in TWO TMEM buffers (step j in buffer j & 1), so the MMA issuer computes S(j+1) and S(j+2)
 // while the softmax group still works on step j: neither side waits for the other in the steady state
 // (with one buffer, S(j+1) cannot start before PV(j) has read the P that overlays S(j), and the chain
 // S -> softmax -> PV -> S leaves the tensor pipe idle half of the time).
@@ -17,14 +17,14 @@
 //               block x 64 columns, addressed through the block table)
 //   warps 10,11 MMA issuer of q-head tile 0 / 1 (one elected lane each): S_t(j) = Q_t·K(j)^T (SS, K-major x K-major, N = 64) into TMEM
 //               buffer j & 1, O_t += P_t(j)·V(j) (P from TMEM [TS] or shared memory [SS], V MN-major); issue
-//               order per step and tile: PV_t(j) S_t(j+2); the two issuers interleave on the tensor pipe
+//               order per step and tile: PV_t(j) S_t(j+2); the two issuers take strict turns on the tensor pipe
 //   warp 8      TMEM allocation (512 columns: O_t at t·D, S_t buffer b at NQ·D + (2t+b)·64; P overlays S)
 //   warps 0-3   softmax of tile 0, warps 4-7 softmax of tile 1: one query row per thread
 //               (tcgen05.ld), causal mask (bottom-right aligned, DESIGN R3), online max with lazy
 //               rescale of O (only when the running max grew by more than 2^8), exp2 with the scale
 //               folded, P -> bf16, row sums in fp32; epilogue O/l -> bf16 -> global.
 // All hand-offs are mbarriers (TMA complete_tx, tcgen05.commit, thread arrivals); the roles of a CTA run
-// decoupled across units (the producer and the MMA warp start the next unit while the softmax groups are in
+// decoupled across units (the producer and the MMA issuers start the next unit while the softmax groups are in
 // the epilogue of the current one).  Tensor-core-bound: algorithmic FLOPs = 4·D·Hq·Σ(q·ctx + q(q+1)/2).
 #pragma once
 #include "pa_common.cuh"
