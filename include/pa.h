@@ -42,8 +42,9 @@
  *       pool[num_blocks][num_kv_heads][block_size = 16][head_dim]     bf16
  *   Logical position t of sequence s lives in slot
  *       (block_tables[s * max_blocks_per_seq + t / 16],  t % 16).
- *   Table entries at index >= ceil(kv_len / 16) are never dereferenced; slots at positions
- *   >= kv_len are never read into a result and never written.
+ *   Table entries at index >= ceil(kv_len / 16) are never used as block ids (the row itself, all
+ *   max_blocks_per_seq entries of it, must be readable: an entry may be loaded ahead of the check that
+ *   discards it); slots at positions >= kv_len are never read into a result and never written.
  *
  * Batch convention: sequences [0, num_decode_seqs) are decode sequences (exactly one new token
  *   each), sequences [num_decode_seqs, n_seq) are prefill chunks (q_len >= 0 new tokens over
