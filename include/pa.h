@@ -194,6 +194,39 @@ int64_t pa_plan_info(const pa_ctx* ctx, int32_t which);
 /* Library-owned message of the last error on ctx (valid until the next call on ctx); "" if none. */
 const char* pa_last_error(const pa_ctx* ctx);
 
+/* ---- Allocation-free decode attention (for callers that cannot call cudaMalloc: code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Needs no pa_ctx, no workspace and no pa_plan.
+ *
+ * pa_decode_attention_static: the decode rows of pa_batch_attention (a5/a6; "Decode attention streams the full
+ * KV-cache context per token") for a batch of n_seq decode sequences, one new token each: token row s
+ * belongs to sequence s and attends to keys 0 .. context_lens[s] (its own KV already appended to the pools):
+ *     out[s][h][:] = softmax_t( softmax_scale * q[s][h] . K_s[t][h / (Hq/Hkv)] ) V_s[t][h / (Hq/Hkv)]
+ * bf16 in, fp32 accumulate, bf16 out; split-KV with the merge in the same launch, by a plain one-warp-per-
+ * (sequence, q head, split) kernel (correct, not tuned: pa_batch_attention is the fast path).
+ *   q, out           dev bf16 [n_seq, Hq, D];  k_pool, v_pool dev bf16 pools (layout above, read only)
+ *   d_context_lens   dev int32 [n_seq];  d_block_tables dev int32 [n_seq, max_blocks_per_seq]
+ *   max_kv_len       host upper bound on context_lens[s] + 1 (only chooses the split count; <= max_blocks_per_seq*16)
+ *   device           CUDA ordinal; must be the calling thread's current device;  stream as for every other call
+ * Scratch: the split partials and the merge's arrival counters live in a file-scope __device__ array of
+ * PA_STATIC_SCRATCH_BYTES that every GPU that loads the library holds until the process exits.  The call calls no
+ * cudaMalloc / cudaFree / allocating routine: it enqueues one cudaMemsetAsync (the counters, which must start at
+ * zero; the array keeps the previous call's contents) and one kernel on `stream`.  The first call on a device also
+ * looks up the array's device address (cudaGetSymbolAddress), so make one call per device outside stream capture.
+ * Size limit: n_seq * Hq * (D*4 + 12) bytes (each of its three pieces rounded up to 256) must fit
+ * PA_STATIC_SCRATCH_BYTES — about 1000 sequences of Hq = 32, D = 128; up to 32 KV splits are used when they fit.
+ * Beyond it: PA_ERR_WORKSPACE, nothing enqueued.  ALL calls on a device share the array: calls that may overlap on the GPU (different streams, or
+ * different host threads without ordering between their streams) race on it; calls on one stream are ordered and safe.
+ * Errors: PA_ERR_INVALID / PA_ERR_UNSUPPORTED (same shape rules as pa_create) / PA_ERR_WORKSPACE / PA_ERR_CUDA;
+ * pa_static_last_error() gives the calling thread's message ("" if its last call succeeded).  n_seq == 0: PA_OK. */
+#define PA_STATIC_SCRATCH_BYTES (16 * 1024 * 1024)
+int32_t pa_decode_attention_static(const void* q, const void* k_pool, const void* v_pool,
+                                   const int32_t* d_context_lens, const int32_t* d_block_tables, int32_t n_seq,
+                                   int32_t num_q_heads, int32_t num_kv_heads, int32_t head_dim,
+                                   int32_t max_blocks_per_seq, int32_t max_kv_len, float softmax_scale, void* out,
+                                   int32_t device, void* stream);
+int64_t pa_static_scratch_bytes(void);        /* = PA_STATIC_SCRATCH_BYTES of the loaded library */
+const char* pa_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

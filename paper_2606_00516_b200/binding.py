@@ -22,7 +22,7 @@ PA_FLAG_PREFILL_P_SMEM = 2
 EXPORTS = ["pa_create", "pa_destroy", "pa_workspace_bytes", "pa_kv_pool_bytes", "pa_kv_append", "pa_plan",
            "pa_batch_attention", "pa_kv_gather", "pa_timer_begin", "pa_timer_end", "pa_timer_record",
            "pa_timer_fit", "pa_timer_kappa", "pa_timer_reset", "pa_crossover_theta0", "pa_crossover_eq7", "pa_plan_info",
-           "pa_last_error"]
+           "pa_last_error", "pa_decode_attention_static", "pa_static_scratch_bytes", "pa_static_last_error"]
 
 
 class PaError(RuntimeError):
@@ -73,8 +73,14 @@ def load_library() -> C.CDLL:
         lib.pa_plan_info.restype = i64
         lib.pa_last_error.argtypes = [vp]
         lib.pa_last_error.restype = C.c_char_p
+        lib.pa_decode_attention_static.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, C.c_float, vp, i32, vp]
+        lib.pa_static_scratch_bytes.argtypes = []
+        lib.pa_static_scratch_bytes.restype = i64
+        lib.pa_static_last_error.argtypes = []
+        lib.pa_static_last_error.restype = C.c_char_p
         for n in EXPORTS:
-            if n not in ("pa_workspace_bytes", "pa_kv_pool_bytes", "pa_plan_info", "pa_last_error"):
+            if n not in ("pa_workspace_bytes", "pa_kv_pool_bytes", "pa_plan_info", "pa_last_error",
+                         "pa_static_scratch_bytes", "pa_static_last_error"):
                 getattr(lib, n).restype = i32
         _lib = lib
     return _lib
@@ -99,6 +105,24 @@ def _stream(stream) -> int:
     if stream is None:
         stream = torch.cuda.current_stream()
     return stream.cuda_stream
+
+
+def decode_attention_static(q, k_pool, v_pool, context_lens, block_tables, max_kv_len: int, softmax_scale: float, out,
+                            stream=None):
+    """pa_decode_attention_static: decode attention with the scratch in the library's static device array (no context,
+    no workspace, no allocation).  q/out [n_seq, Hq, D] bf16; pools [num_blocks, Hkv, 16, D]; block_tables
+    [n_seq, max_blocks_per_seq] int32; all on the current CUDA device."""
+    lib = load_library()
+    n_seq, hq, d = q.shape
+    rc = lib.pa_decode_attention_static(_ptr(q), _ptr(k_pool), _ptr(v_pool), _ptr(context_lens), _ptr(block_tables),
+                                        n_seq, hq, k_pool.shape[1], d, block_tables.shape[1], max_kv_len,
+                                        C.c_float(softmax_scale), _ptr(out), q.device.index, _stream(stream))
+    if rc != PA_OK:
+        raise PaError(rc, lib.pa_static_last_error().decode())
+
+
+def static_scratch_bytes() -> int:
+    return int(load_library().pa_static_scratch_bytes())
 
 
 class PagedAttention:
