@@ -19,8 +19,6 @@
 //   an item that covers a whole (seq, head) writes its output rows directly; split groups write
 //     (m, l, o) partials and the LAST arriving consumer merges them (m = max m_i, l = Σ l_i 2^{m_i-m},
 //     o = Σ o_i 2^{m_i-m} / l) — one launch, no separate merge kernel.
-// Every mbarrier wait of this role first asks with test_wait (mbar_wait_likely_done): with short items the phase
-// is complete more often than not, and try_wait costs ~100 cycles even then (C2 r = 1: 52 -> 44 us).
 // HBM-bound: algorithmic bytes per decode token = kv_len·kvb + 2·qb + 4·ceil(kv_len/16).
 #pragma once
 #include "pa_common.cuh"
@@ -187,7 +185,7 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
         {
             const uint32_t fs = i_iss % FQ;
             if (threadIdx.x == 0) PA_TL(1, (int)i_iss, 0);
-            mbar_wait_likely_done(bar + Cfg::kOffFEmpty + 8 * fs, ((i_iss / FQ) & 1u) ^ 1u);
+            mbar_wait(bar + Cfg::kOffFEmpty + 8 * fs, ((i_iss / FQ) & 1u) ^ 1u);
             if (threadIdx.x == 0) PA_TL(1, (int)i_iss, 1);
             const uint32_t d = smem_u32(aux + Cfg::kOffDesc + 32 * fs);
             asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(d), "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w) : "memory");
@@ -213,7 +211,7 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
 #pragma unroll
                 for (int h = 0; h < H; ++h) {
                     const uint32_t slot = u_iss % R;
-                    mbar_wait_likely_done(bar + Cfg::kOffEmpty + 8 * slot, ((u_iss / R) & 1u) ^ 1u);
+                    mbar_wait(bar + Cfg::kOffEmpty + 8 * slot, ((u_iss / R) & 1u) ^ 1u);
                     const uint32_t full = bar + 8 * slot, dst = ring_u32 + slot * Cfg::kUnit;
                     if (nvalid == kBlock) {
                         mbar_expect_tx(full, Cfg::kUnit);
@@ -243,7 +241,7 @@ __device__ __forceinline__ void decode_producer(const AttnParams& p, const CUten
     // ---- sentinel item: tells the consumer that the stream is finished
     {
         const uint32_t fs = i_iss % FQ;
-        mbar_wait_likely_done(bar + Cfg::kOffFEmpty + 8 * fs, ((i_iss / FQ) & 1u) ^ 1u);
+        mbar_wait(bar + Cfg::kOffFEmpty + 8 * fs, ((i_iss / FQ) & 1u) ^ 1u);
         const uint32_t d = smem_u32(aux + Cfg::kOffDesc + 32 * fs);
         asm volatile("st.shared.b32 [%0], %1;" ::"r"(d), "r"(-1) : "memory");
         mbar_arrive(bar + Cfg::kOffFFull + 8 * fs);
@@ -369,7 +367,7 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
     for (;;) {
         const uint32_t fs = i_con % FQ;
         if (threadIdx.x == 128) PA_TL(0, (int)i_con, 0);
-        mbar_wait_likely_done(bar + Cfg::kOffFFull + 8 * fs, (i_con / FQ) & 1u);
+        mbar_wait(bar + Cfg::kOffFFull + 8 * fs, (i_con / FQ) & 1u);
         if (threadIdx.x == 128) PA_TL(0, (int)i_con, 1);
         const DecItem ci = *reinterpret_cast<const DecItem*>(aux + Cfg::kOffDesc + 32 * fs);
         if (ci.seq < 0) break;
@@ -395,8 +393,8 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
                 float sB0[4] = {0.f, 0.f, 0.f, 0.f}, sB1[4] = {0.f, 0.f, 0.f, 0.f};
                 const uint32_t tKA = ring_u32 + sKA * Cfg::kUnit, tKB = ring_u32 + sKB * Cfg::kUnit;
                 const uint32_t rowk = r8 + 8 * (mi & 1);
-                mbar_wait_likely_done(bar + 8 * sKA, phKA);
-                mbar_wait_likely_done(bar + 8 * sKB, phKB);
+                mbar_wait(bar + 8 * sKA, phKA);
+                mbar_wait(bar + 8 * sKB, phKB);
                 if (threadIdx.x == 128) PA_TL(2, (int)i_con, 0);
 #pragma unroll
                 for (int k2 = 0; k2 < 4; ++k2) {
@@ -446,8 +444,8 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
                 const uint32_t tVA = ring_u32 + sVA * Cfg::kUnit, tVB = ring_u32 + sVB * Cfg::kUnit;
                 const uint32_t rowv = r8 + 8 * (mi >> 1);
                 if (threadIdx.x == 128) PA_TL(2, (int)i_con, 2);
-                mbar_wait_likely_done(bar + 8 * sVA, phVA);
-                mbar_wait_likely_done(bar + 8 * sVB, phVB);
+                mbar_wait(bar + 8 * sVA, phVA);
+                mbar_wait(bar + 8 * sVB, phVB);
                 if (threadIdx.x == 128) PA_TL(2, (int)i_con, 3);
                 if (nvalidB < 16) decode_zero_dead_rows(tVB, nvalidB, lane);
                 if (threadIdx.x == 128) PA_TL(3, (int)i_con, 0);
@@ -478,7 +476,7 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
 #pragma unroll
             for (int h = 0; h < H; ++h) {
                 const uint32_t slot = u_con % R;
-                mbar_wait_likely_done(bar + 8 * slot, (u_con / R) & 1u);
+                mbar_wait(bar + 8 * slot, (u_con / R) & 1u);
                 const uint32_t tile = ring_u32 + slot * Cfg::kUnit;
                 const uint32_t row = r8 + 8 * (mi & 1);
 #pragma unroll
@@ -528,7 +526,7 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
 #pragma unroll
             for (int h = 0; h < H; ++h) {
                 const uint32_t slot = u_con % R;
-                mbar_wait_likely_done(bar + 8 * slot, (u_con / R) & 1u);
+                mbar_wait(bar + 8 * slot, (u_con / R) & 1u);
                 const uint32_t tile = ring_u32 + slot * Cfg::kUnit;
                 if (nvalid < 16) decode_zero_dead_rows(tile, nvalid, lane);
                 const uint32_t row = r8 + 8 * (mi >> 1);               // token
