@@ -100,6 +100,26 @@ def test_attention_parity_small(name, mode):
     gc.check_close(sdev.bits(d["out"]), ref, f"{name}/mode{mode}")
 
 
+@pytest.mark.parametrize("seed", range(300, 314))
+def test_random_shapes_and_mixes(seed):
+    """Shapes and mixes nobody picked by hand: head_dim, KV heads, group size 1..8, decode / prefill counts and length
+    ranges are all drawn from the seed; every row against the oracle, pools bit-exact, alternating launch orders."""
+    rng = np.random.default_rng(seed)
+    d = int(rng.choice([128, 256]))
+    hkv = int(rng.choice([1, 2, 4, 8]))
+    g = int(rng.integers(1, min(8, 32 // hkv) + 1))
+    n_dec, n_pre = int(rng.integers(0, 48)), int(rng.integers(0, 4))
+    if n_dec + n_pre == 0:
+        n_dec = 1
+    batch = workloads.random_batch(seed, workloads.Shape(hkv * g, hkv, d), n_dec, n_pre,
+                                   max_ctx=int(rng.choice([40, 300, 1500])), max_q=int(rng.choice([20, 130, 300])))
+    inp = helpers.host_inputs(batch)
+    dd = gc.run_gpu(batch, inp, flags=(0, binding.PA_FLAG_PREFILL_P_SMEM)[seed % 3 == 0], order=("plan_first", "graph")[seed % 2])
+    ref, kp, vp = gc.run_oracle(batch, inp)
+    assert (sdev.bits(dd["k_pool"]) == kp).all() and (sdev.bits(dd["v_pool"]) == vp).all(), "pools differ after append"
+    gc.check_close(sdev.bits(dd["out"]), ref, f"fuzz seed {seed}: Hq {hkv * g} Hkv {hkv} D {d}, {n_dec} decode + {n_pre} prefill")
+
+
 @pytest.mark.parametrize("order", ["plan_between", "graph"])
 @pytest.mark.parametrize("name", ["C1", "ragged-g4-d128", "ragged-g4-d256", "edge-lens", "decode-only", "prefill-only"])
 def test_call_orders_small(name, order):
