@@ -545,6 +545,7 @@ __device__ __forceinline__ void decode_consumer(const AttnParams& p, uint8_t* st
         }
         // ---------------- item finished
         if (threadIdx.x == 128) PA_TL(0, (int)i_con, 2);
+        if (lane == 0) PA_TL_CTA(3);        // (instrumented build only) the CTA's latest "blocks of an item consumed"
         ++i_con;
 #pragma unroll
         for (int off = 4; off <= 16; off <<= 1) {
