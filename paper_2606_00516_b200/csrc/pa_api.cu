@@ -441,27 +441,29 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
     int k = 0, levels = 1;
     if (total_blocks > 0) {
         // workers that start in the decode role; in a mixed launch the prefill CTAs join through the queue when
-        // their units run out, so bundles are made finer (>= 2 per worker) and the tail balances dynamically
+        // their units run out (if the rule below leaves bundles in the queue)
         const int64_t W = (int64_t)(sms - pre_ctas) * kDecodeWarps;
         // Bundles per worker (measured on B200): pure decode — one static bundle per stream is best up to a few GB of
         // KV (every extra cut adds parts to the in-launch merges: 4 sequences x 128k keys run at 0.95 of the HBM
         // roofline with 1 bundle per worker and 0.57 with 4); from ~16 GB on a launch lasts milliseconds and a second,
-        // queue-drawn bundle per worker evens out unequal stream rates (C5: -5 %).  Mixed launches: 2 per worker (below).
+        // queue-drawn bundle per worker evens out unequal stream rates (C5: -5 %).
         const double kv_bytes = (double)total_blocks * kBlock * D * 2 * 2;
         // (C5 on one B200, same call, interleaved, median [min, max] over 24 launches: k = 1 6.47 [5.87, 6.81] ms,
         // k = 2 6.67 [5.81, 6.90], k = 3 5.86 [5.81, 5.91], k = 4 6.31 [6.22, 6.41]: three per stream from 16 GB on.)
-        // A launch whose prefill role takes one or two CTAs is a decode launch for this purpose: nothing is lost when
-        // those CTAs find the queue empty, and two equal queue-drawn bundles per stream leave a tail of up to half a
-        // share when a fast stream takes a third one (Table-9-shaped batches, n_tok 2048, r = 0.5 / 0.9, same call,
-        // three rounds each: k = 2 1760-1800 us or 1600 us depending on the run, k = 1 1558-1564 us; 740-840 vs 731).
-        k = kv_bytes >= 16e9 ? 3 : (pre_ctas > 2 ? 2 : 1);
-        // Ragged batches of many groups per stream (>= 4: C4-shaped, lognormal contexts) already gain from three
-        // bundles per stream at 8 GB when the prefill role is small (bench.py protocol, same call, k = 1 / 2 / 3):
-        // 1024 decode sequences, 10.6 GB: 1977 / 1666 / 1584 us; n_tok 1024 r = 0.8, 8.4 GB: 1605 / 1417 / 1241;
-        // n_tok 2048 r = 0.6, 12.6 GB: 2438 / 1994 / 1868.  Batches of a few long, equal sequences (under one group per
-        // stream) run at the read ceiling with one static bundle and lose 0-7 % with three, so they keep k = 1.
+        // The rule below is the best, or within 1 % of the best, of k = 1, 2, 3 on every configuration swept under
+        // bench.py's timing protocol at the end of round 2 (DESIGN.md §6.5 has the table):
+        //  - two equal queue-drawn halves per stream (k = 2) leave a tail of up to half a share when a fast stream
+        //    takes a third one, and which stream does differs from run to run (same plan: 1600 or 1780 us), so k = 2 is
+        //    only used where late-joining prefill CTAs need queue-drawn work: > 2 prefill CTAs and >= 4.5 GB of KV
+        //    (below that one static bundle per stream is as fast or faster: 3.3 GB 587 -> 518 us, 4.4 GB 712 -> 666);
+        //  - ragged batches of >= 3 groups per stream (C4-shaped, lognormal contexts) with a small prefill role take
+        //    three bundles per stream from 5 GB on (k = 1 / 2 / 3: 10.6 GB 1977 / 1666 / 1584 us; 12.6 GB 2438 / 1994 /
+        //    1868; 8.4 GB 1605 / 1417 / 1241; 5.2 GB 879 / 872 / 839), everything from 16 GB on;
+        //  - batches of a few long, equal sequences (under one group per stream) run at the read ceiling with one static
+        //    bundle per stream and lose 0-7 % with three, so they keep k = 1 up to 16 GB.
         const double groups_per_share = (double)n_dec * Hkv / (double)W;
-        if (kv_bytes >= 8e9 && groups_per_share >= 4.0 && pre_ctas <= 4) k = 3;
+        k = (pre_ctas > 2 && kv_bytes >= 4.5e9) ? 2 : 1;
+        if (kv_bytes >= 16e9 || (kv_bytes >= 5e9 && groups_per_share >= 3.0 && pre_ctas <= 4)) k = 3;
         // Guided hand-out (PlanView::n_levels): when a stream's share holds many groups (>= 16) and the launch is long
         // enough for unequal stream rates to matter (>= 1 GB of KV, ~150 us), the bundles (two per stream) are taken in
         // eight pieces of 50, 20, 12, 7, 5, 3, 2, 1 % of their groups, large pieces first.  With whole bundles every
