@@ -442,7 +442,11 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
             pre_ctas = (int32_t)std::lround(std::min<double>(need, sms - 96));
             pre_ctas = std::max(pre_ctas, (int32_t)std::lround(sms * t_pre / (t_pre + sms * t_hbm)));
         } else {
-            pre_ctas = (int32_t)std::lround(sms * t_pre / (t_pre + t_lat));
+            // latency-bound launches (C2): the per-unit figures above are round-1 measurements and the prefill role
+            // has become faster since; with 0.65 of them the two roles finish together (C2 r = 0.1 ... 0.9, attention
+            // launch with factor 1 / 0.8 / 0.64: 38.9 / 35.8 / 33.8, -- / 37.8 / 34.9, 41.9 / 39.0 / 37.9, -- / 39.4 / 38.9,
+            // 43.1 / 42.0 / 39.9, -- / 43.9 / 43.0, 46.1 / 46.0 / 44.5, -- / 47.9 / 48.1, 50.1 / 48.2 / 48.1 us)
+            pre_ctas = (int32_t)std::lround(sms * 0.65 * t_pre / (0.65 * t_pre + t_lat));
         }
         if (c.tune_prefill_ctas > 0) pre_ctas = c.tune_prefill_ctas;
         pre_ctas = std::max(1, std::min({pre_ctas, sms - 1, n_units}));
