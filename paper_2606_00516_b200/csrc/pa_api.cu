@@ -497,6 +497,10 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
         const int64_t min_blocks = c.tune_min_bundle_blocks > 0 ? c.tune_min_bundle_blocks : 2;
         bc.target = std::max(min_blocks, (total_blocks + W * k - 1) / (W * k));
         bc.use_carry = k == 1;
+        // One static bundle per stream must not leave a bundle over: it would run as a second wave on one stream.  The
+        // carried rounding keeps the count within one of the stream count; if it still comes out above, cut again with
+        // a slightly larger target (rare; one more O(bundles) pass).
+        for (int attempt = 0;; ++attempt) {
         for (int s = 0; s < n_dec && !bc.overflow; ++s) {
             const int32_t nblk = (h_ctx[s] + kBlock) / kBlock;          // ceil((ctx + 1) / 16)
             const int32_t grp0 = s * Hkv;
@@ -540,6 +544,11 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
             }
         }
         bc.close();
+        if (k != 1 || bc.overflow || bc.n_bundles <= W || attempt == 3) break;
+        const int64_t wider = bc.target + std::max<int64_t>(1, bc.target / 32);
+        bc = BundleCutter{bc.out, bc.max_bundles, bc.max_split, wider};
+        bc.use_carry = true;
+        }
         if (bc.overflow) return fail(ctx, PA_ERR_INVALID, "pa_plan: decode bundle / partial-slot list overflow");
     }
     const int32_t n_bundles = bc.n_bundles;

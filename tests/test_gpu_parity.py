@@ -120,6 +120,30 @@ def test_random_shapes_and_mixes(seed):
     gc.check_close(sdev.bits(dd["out"]), ref, f"fuzz seed {seed}: Hq {hkv * g} Hkv {hkv} D {d}, {n_dec} decode + {n_pre} prefill")
 
 
+def test_one_bundle_per_stream_leaves_none_over():
+    """Planner (host logic, needs a device only for the upload): with one static bundle per stream no bundle may be left
+    over for a second wave, whatever the mix of short (uncut) and long groups; checked on 80 seed-drawn batches (plans only)."""
+    rng = np.random.default_rng(4242)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    seen_k1 = 0
+    for i in range(80):
+        hkv = int(rng.choice([1, 2, 4, 8]))
+        shape = workloads.Shape(hkv * int(rng.integers(1, 5)), hkv, int(rng.choice([128, 256])))
+        n_dec = int(rng.integers(200, 3000))
+        ctx_hi = int(rng.choice([16, 40, 128, 300, 700]))
+        n_pre = int(rng.integers(0, 3))
+        batch = workloads.random_batch(5000 + i, shape, n_dec, n_pre, max_ctx=ctx_hi, max_q=200)
+        pa = gc.make_ctx(batch)
+        pa.plan(batch.cu_seqlens_q, batch.context_lens, batch.n_seq, batch.num_decode_seqs)
+        if pa.plan_info(7) == 1 and pa.plan_info(10) == 1:
+            seen_k1 += 1
+            streams = (sms - pa.plan_info(6)) * 8
+            assert pa.plan_info(1) <= streams, (f"batch {i}: {pa.plan_info(1)} bundles for {streams} streams "
+                                                f"({n_dec} decode seqs, ctx <= {ctx_hi}, Hkv {hkv})")
+        pa.close()
+    assert seen_k1 >= 40
+
+
 @pytest.mark.parametrize("order", ["plan_between", "graph"])
 @pytest.mark.parametrize("name", ["C1", "ragged-g4-d128", "ragged-g4-d256", "edge-lens", "decode-only", "prefill-only"])
 def test_call_orders_small(name, order):
