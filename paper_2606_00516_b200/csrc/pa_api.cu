@@ -471,16 +471,23 @@ int32_t pa_plan(pa_ctx* ctx, const int32_t* h_cu, const int32_t* h_ctx, int32_t 
         // The rule below is the best, or within 1 % of the best, of k = 1, 2, 3 on every configuration swept under
         // bench.py's timing protocol at the end of round 2 (DESIGN.md §6.5 has the table):
         //  - two equal queue-drawn halves per stream (k = 2) leave a tail of up to half a share when a fast stream
-        //    takes a third one, and which stream does differs from run to run (same plan: 1600 or 1780 us), so k = 2 is
-        //    only used where late-joining prefill CTAs need queue-drawn work: > 2 prefill CTAs and >= 4.5 GB of KV
-        //    (below that one static bundle per stream is as fast or faster: 3.3 GB 587 -> 518 us, 4.4 GB 712 -> 666);
+        //    takes a third one, and which stream does differs from run to run (same plan: 1600 or 1780 us); mixed
+        //    launches (> 2 prefill CTAs) take thirds from 4.5 GB of KV on so that late-joining prefill CTAs find
+        //    queue-drawn work (below that one static bundle per stream is as fast or faster: 3.3 GB 587 -> 518 us,
+        //    4.4 GB 712 -> 666);
         //  - ragged batches of >= 3 groups per stream (C4-shaped, lognormal contexts) with a small prefill role take
         //    three bundles per stream from 5 GB on (k = 1 / 2 / 3: 10.6 GB 1977 / 1666 / 1584 us; 12.6 GB 2438 / 1994 /
         //    1868; 8.4 GB 1605 / 1417 / 1241; 5.2 GB 879 / 872 / 839), everything from 16 GB on;
         //  - batches of a few long, equal sequences (under one group per stream) run at the read ceiling with one static
         //    bundle per stream and lose 0-7 % with three, so they keep k = 1 up to 16 GB.
         const double groups_per_share = (double)n_dec * Hkv / (double)W;
-        k = (pre_ctas > 2 && kv_bytes >= 4.5e9) ? 2 : 1;
+        // (mixed, >= 4.5 GB: halves or thirds by groups per stream — five fresh processes each, k = 2 / 3: 4.5 groups per
+        // stream 1133-1148 / 992-1007 us, 5.9: 1420-1433 / 1275-1278, 6.1: 1338-1340 / 1343-1346, 7.9: 1342-1357 / 1346-1358,
+        // 8.8: 1974-1987 / 2120)
+        // Halves are not used at all (outside the guided hand-out): the same k = 2 plan of the headline's r = 0.1 batch ran
+        // at 1342-1357 us in five processes and at 1480 us in a sixth, thirds at 1346-1358 in all; with >= 8.5 groups per
+        // stream one static bundle (with the carried rounding) is as fast as halves (1989-2000 vs 1974-1987 us).
+        k = (pre_ctas > 2 && kv_bytes >= 4.5e9 && groups_per_share < 8.5) ? 3 : 1;
         if (kv_bytes >= 16e9 || (kv_bytes >= 5e9 && groups_per_share >= 3.0 && pre_ctas <= 4)) k = 3;
         // Guided hand-out (PlanView::n_levels): when a stream's share holds many groups (>= 16) and the launch is long
         // enough for unequal stream rates to matter (>= 1 GB of KV, ~150 us), the bundles (two per stream) are taken in
